@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Kratos hydro hot path on B200 (cell-updates/s and % of HBM roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload C5|C4|C3|C5-256] [--precision mixed|fp64]
+
+A "step" is one full Heun step (both stages: ghost rules, primitive recovery, PLM, HLLC, fp64 update,
+fused CFL reduction) of one synthetic block.  Default workload: BASELINE.json config 5 (512^3 periodic,
+gamma 1.001, Mach-1 random-phase velocity field, mixed precision) -- the configuration the metric is
+quoted on.  Prints ONE JSON line (rank 0).
+
+Multi-GPU: the path does not shard in this build (BASELINE.json: one GPU, no collectives), so
+--gpus N runs N independent replicas ("replicas only"); torch.distributed is
+used for the barrier and the max-over-ranks time only.
+
+--impl reference times the oracle (oracle/kratos_oracle.c, as it stands) on the host cores on a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/sec per B200 (3D hydro step) and % of HBM roofline"
+UNIT = "cell-updates/s"
+BYTES_PER_CELL = {"stage1": 80.0, "stage2": 120.0}  # algorithmic HBM bytes per cell
+
+
+def workload(name: str):
+    from paper_2501_02317_b200 import inputs
+    if name == "C5":
+        return inputs.turbulence_3d(512, seed=5, nsteps=20), "C5 3D decaying turbulence 512^3 periodic gamma=1.001"
+    if name == "C5-256":
+        return inputs.turbulence_3d(256, seed=5, nsteps=20), "C5 recipe at 256^3"
+    if name == "C5-128":
+        return inputs.turbulence_3d(128, seed=5, nsteps=20), "C5 recipe at 128^3"
+    if name == "C4":
+        return inputs.point_blast_3d(256, nsteps=50), "C4 3D point blast 256^3 outflow gamma=5/3"
+    if name == "C3":
+        return inputs.shear_layer_2d(2048, seed=3, nsteps=100), "C3 2D shear layer 2048^2 periodic gamma=5/3"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload_name: str, precision: str):
+    """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this workload."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            return json.load(f).get(f"{workload_name}:{precision}")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [l for (t, l) in self.lines if t0 - 0.05 <= t <= t1 + 0.15] or [l for (_, l) in self.lines]
+        sm, mx, reasons = [], [], set()
+        for l in rows:
+            p = [x.strip() for x in l.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(pr_small, steps: int, warmup: int):
+    """Oracle on the host cores: `steps` Heun steps (incl. its own CFL pass) of a bounded sample."""
+    import oracle
+    U = pr_small.U.copy()
+    for _ in range(warmup):
+        oracle.run(U, pr_small.gamma, pr_small.bc, pr_small.cfl, 1)
+    t0 = time.time()
+    oracle.run(U, pr_small.gamma, pr_small.bc, pr_small.cfl, steps)
+    dt = time.time() - t0
+    return pr_small.ncell * steps / dt, dt, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2501_02317_b200 import inputs
+    n = 96
+    pr = inputs.turbulence_3d(n, seed=5) if args.workload.startswith("C5") else workload(args.workload)[0]
+    sample = f"C5 recipe at {n}^3, {args.steps} timed Heun steps after {args.warmup} warm-up (oracle as it stands, OpenMP)"
+    if not args.workload.startswith("C5"):
+        sample = f"{pr.name} full size, {args.steps} steps"
+    value, dt, cores = time_oracle(pr, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload(args.workload)[1] if args.workload != "C5" else
+                   "C5 3D decaying turbulence 512^3 periodic gamma=1.001", "precision": "fp64 (oracle)",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2501_02317_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    pr, wl_name = workload(args.workload)
+    prec = binding.PREC_MIXED if args.precision == "mixed" else binding.PREC_FP64
+    nx, ny, nz = pr.shape
+    ncell = pr.ncell
+    stream = torch.cuda.Stream()
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream)
+    host = torch.from_numpy(pr.U).pin_memory()            # pinned host copy (e2e leg)
+    with torch.cuda.stream(stream):
+        dev = host.to("cuda", non_blocking=True)
+        h.set_state(dev)
+        stream.synchronize()
+        del dev
+
+        def barrier():
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        # ---- device-resident throughput -------------------------------------------------------
+        t = h.run(pr.cfl, args.warmup, 0.0)
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        time.sleep(0.25)
+        barrier()
+        h.set_profiling(True)
+        l0 = h.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0 = time.time()
+        e0.record(stream)
+        t = h.run(pr.cfl, args.steps, t)
+        e1.record(stream)
+        barrier()
+        w1 = time.time()
+        ms = e0.elapsed_time(e1)
+        launches = h.launch_count() - l0
+        timing = h.get_timing()
+        h.set_profiling(False)
+        clocks = sampler.stop(w0, w1)
+        if dist is not None:
+            tt = torch.tensor([ms], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ms = float(tt.item())
+        value = ncell * world * args.steps / (ms * 1e-3)
+        hits = h.floor_hits()
+
+        # ---- end to end: host buffers through the C-ABI, copies inside the timed region -------
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        h.set_state(host)
+        h.run(pr.cfl, 1, 0.0)
+        h.get_state(host)
+        barrier()
+        w2 = time.time()
+        te = 0.0
+        for _ in range(e2e_steps):
+            h.set_state(host)          # H2D of this step's input from pinned memory (5 N doubles)
+            te = h.run(pr.cfl, 1, te)  # one Heun step (its CFL pass included: fresh state)
+            h.get_state(host)          # D2H of the step's result
+        barrier()
+        e2e_s = time.time() - w2
+        if dist is not None:
+            tt = torch.tensor([e2e_s], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_s = float(tt.item())
+        e2e_value = ncell * world * e2e_steps / e2e_s
+    h.destroy()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peak()
+    kern = {}
+    for k in ("stage1", "stage2"):
+        tot_ms, n = timing[k]
+        if n:
+            avg = tot_ms / n
+            gbs = BYTES_PER_CELL[k] * ncell / (avg * 1e-3) / 1e9
+            kern[k] = {"avg_ms": avg, "launches": n, "algorithmic_bytes": BYTES_PER_CELL[k] * ncell,
+                       "achieved_gbs": gbs, "frac": gbs / peak}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
+    roofline = None
+    if dom:
+        roofline = {"bound": "hbm", "kernel": f"stage_tiled<{'float' if prec == 0 else 'double'},{dom[-1]},3>"
+                    if nz > 1 else f"stage_tiled<...,{dom[-1]},2>",
+                    "achieved": kern[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": kern[dom]["frac"], "traffic": ncu_traffic(args.workload, args.precision),
+                    "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL[dom]}
+    step_frac = value / world * 200.0 / (peak * 1e9)
+
+    # ---- oracle on the host cores, bounded sample (rank 0, N = 1 only) ---------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s = 128 if nz > 1 else 1024
+        small = inputs.turbulence_3d(n_s, seed=5) if nz > 1 else inputs.shear_layer_2d(n_s, seed=3)
+        v, dt_s, cores = time_oracle(small, 2, 0)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{small.name} recipe at {n_s}^{3 if nz > 1 else 2}, 2 Heun steps ({dt_s:.1f} s)"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32 flux / f64 state" if prec == 0 else "f64", "data": "synthetic",
+        "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": args.precision,
+                   "scheme": "PLM-minmod + HLLC + Heun", "cfl": pr.cfl, "parallelism": f"replicas x{world}",
+                   "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
+                   if 40 * ncell > 2.5e8 else "state fits L2: no flush between steps (steps are data-dependent)",
+                   "floor_hits": hits},
+        "hbm_roofline_frac_step": step_frac,
+        "roofline": roofline, "kernels": kern, "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * ncell, "d2h_bytes_per_step": 40 * ncell,
+                "steps": e2e_steps},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5")
+    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,151 @@
+/*
+ * kratos_hydro.h -- C-ABI boundary of the B200-native Kratos hydrodynamics hot path.
+ *
+ * The library advances the compressible Euler equations (Eq. 2)
+ *     d_t rho + div(rho v) = 0,  d_t(rho v) + div(rho v v + p I) = 0,  d_t eps + div[(eps+p) v] = 0,
+ *     eps = p/(gamma-1) + rho v^2/2
+ * on ONE uniform Cartesian block on ONE GPU with the paper's default scheme: primitive
+ * recovery (Sec. 3.1), ghost zones by the paper's boundary rules
+ * (Sec. 3.1.1), minmod-limited PLM (Eq. 3), the
+ * subtraction-safe HLLC solver (Eq. 4-5), a flux-difference update inside
+ * the Heun integrator (Sec. 3.3), the CFL time-step reduction
+ * and the mixed-precision split float_t / float2_t (Sec. 3.2.2,
+ * PAPER.md:230-240).  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU
+ * fallback: without a CUDA device every call that computes fails with KRATOS_ERR_CUDA.
+ *
+ * Conventions
+ *  - State layout: conserved U = (rho, m_x, m_y, m_z, eps), struct of arrays
+ *    U[5][nz][ny][nx] of double, x fastest, INTERIOR cells only (the library keeps no ghost
+ *    storage: boundary rules are applied as the stencil is loaded).
+ *  - An axis is active when its extent is > 1 (nz = 1: 2D, ny = nz = 1: 1D).  Active axes
+ *    need extent >= 4.  Inactive axes carry no flux; their bc entries are ignored and their
+ *    momentum stays exactly as given (normally 0).
+ *  - Cell centres x_i = (i + 1/2) dx; default spacing 1/n per active axis (unit box).
+ *  - Every function returning int returns KRATOS_OK (0) or a negative error code; the message
+ *    is available from kratos_hydro_last_error() (thread-local).  The handle owns all device
+ *    memory; the caller owns every buffer it passes.  A handle is not thread-safe.
+ *  - "host"/"device" below says where a pointer must live.  Device pointers must belong to
+ *    the current CUDA device of the calling thread at create time.
+ *  - All work is enqueued on the stream given by kratos_hydro_set_stream (default: the
+ *    legacy default stream 0).  Calls documented as "asynchronous" return before the GPU
+ *    has finished; all others synchronise that stream before returning.
+ */
+#ifndef KRATOS_HYDRO_H
+#define KRATOS_HYDRO_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define KRATOS_API __attribute__((visibility("default")))
+#else
+#define KRATOS_API
+#endif
+
+typedef struct kratos_hydro kratos_hydro_t; /* opaque */
+
+/* error codes */
+#define KRATOS_OK 0
+#define KRATOS_ERR_ARG (-1)       /* bad argument (see each call) */
+#define KRATOS_ERR_ALLOC (-2)     /* device or host allocation failed */
+#define KRATOS_ERR_CUDA (-3)      /* CUDA runtime error / no device */
+#define KRATOS_ERR_NONFINITE (-4) /* non-finite state or time step detected */
+
+/* scheme word: bits 0-1 precision, bits 4-5 integrator.
+ * Reconstruction is PLM-minmod and the Riemann solver HLLC (the paper's defaults; no other choice). */
+#define KRATOS_PREC_MIXED 0 /* float_t = fp32 (reconstruction, Riemann), float2_t = fp64 (state, update) */
+#define KRATOS_PREC_FP64 1  /* float_t = float2_t = fp64 */
+#define KRATOS_INTEGRATOR_HEUN (0 << 4)
+
+/* boundary codes, the paper's list order */
+#define KRATOS_BC_PERIODIC 0 /* communication boundary onto the same block: wrap copy */
+#define KRATOS_BC_FREE 1     /* q(-i-1/2) = q(1/2) */
+#define KRATOS_BC_OUTFLOW 2  /* Free, but inward normal velocity v(-i-1/2) = min(v(1/2), 0) */
+#define KRATOS_BC_REFLECT 3  /* q(-i-1/2) = q(i+1/2), normal velocity negated */
+
+/* kernel variants (kratos_hydro_set_kernel) */
+#define KRATOS_KERNEL_AUTO 0   /* tiled where supported (x,y active), else simple */
+#define KRATOS_KERNEL_SIMPLE 1 /* one thread per cell, stencil from global memory (any axes) */
+#define KRATOS_KERNEL_TILED 2  /* shared-memory tile + halo, z marched in registers, each face once */
+
+/* Create a solver for an nx*ny*nz block.  gamma > 1.  bc (host, 6 ints) =
+ * {x-lo, x-hi, y-lo, y-hi, z-lo, z-hi}; periodic must be set on both sides of an axis or
+ * neither.  Allocates two copies of the state plus small work buffers on the current device.
+ * Returns NULL on error (bad argument, no device, out of memory): see kratos_hydro_last_error(). */
+KRATOS_API kratos_hydro_t *kratos_hydro_create(int nx, int ny, int nz, double gamma, int scheme, const int bc[6]);
+
+/* Free everything the handle owns.  NULL is allowed. */
+KRATOS_API void kratos_hydro_destroy(kratos_hydro_t *h);
+
+/* Cell sizes (> 0, finite); entries of inactive axes are ignored.  Default 1/n. */
+KRATOS_API int kratos_hydro_set_spacing(kratos_hydro_t *h, double dx, double dy, double dz);
+
+/* Stream (a cudaStream_t passed as void*) used by all later calls.  The caller keeps ownership. */
+KRATOS_API int kratos_hydro_set_stream(kratos_hydro_t *h, void *cuda_stream);
+
+/* Choose the kernel variant (KRATOS_KERNEL_*).  KRATOS_ERR_ARG if the variant does not
+ * support this block's active axes. */
+KRATOS_API int kratos_hydro_set_kernel(kratos_hydro_t *h, int variant);
+
+/* z-extent of the slab one thread block of the tiled kernel marches through (0 = automatic). */
+KRATOS_API int kratos_hydro_set_zchunk(kratos_hydro_t *h, int planes);
+
+/* Copy a state in.  U: 5*nx*ny*nz doubles in the layout above; on_device = 0: host pointer
+ * (pageable or pinned), 1: device pointer.  Synchronises the stream when U is on the host. */
+KRATOS_API int kratos_hydro_set_state(kratos_hydro_t *h, const double *U, int on_device);
+
+/* Copy the current state out (same layout and rules).  KRATOS_ERR_NONFINITE is NOT checked here. */
+KRATOS_API int kratos_hydro_get_state(kratos_hydro_t *h, double *U, int on_device);
+
+/* CFL time step of the current state:
+ *   dt = cfl / max_cells sum_{active d} (|v_d| + c)/dx_d,  c = sqrt(gamma p / rho),
+ * evaluated in fp64 in every precision mode by a min-reduction kernel.  dt_out: host.
+ * Synchronises.  KRATOS_ERR_NONFINITE if the result is not finite and positive. */
+KRATOS_API int kratos_hydro_cfl_dt(kratos_hydro_t *h, double cfl, double *dt_out);
+
+/* One full Heun step of length dt (> 0, finite; else KRATOS_ERR_ARG):
+ *   U1 = U + dt L(U);  U <- 1/2 U + 1/2 (U1 + dt L(U1))
+ * Asynchronous. */
+KRATOS_API int kratos_hydro_step(kratos_hydro_t *h, double dt);
+
+/* nsteps Heun steps with the time step kept on the device (no host round trip per step):
+ * before each step dt = cfl / (rate maximum of the current state), the maximum having been
+ * reduced inside the previous step's final kernel (first step: by the cfl_dt kernel).  In mixed
+ * precision that fused rate is evaluated in float_t from the freshly updated float2_t state.
+ * t_inout (host): time before / after.  Synchronises at the end. */
+KRATOS_API int kratos_hydro_run(kratos_hydro_t *h, double cfl, int nsteps, double *t_inout);
+
+/* As run, but every dt is clipped so that t lands exactly on t_end; stops when t == t_end or
+ * after max_steps.  steps_done (host, may be NULL). */
+KRATOS_API int kratos_hydro_run_until(kratos_hydro_t *h, double cfl, double t_end, int max_steps,
+                           double *t_inout, int *steps_done);
+
+/* Compensated (double-double) sums of the five conserved fields over the interior, not
+ * multiplied by the cell volume.  out: host.  Synchronises. */
+KRATOS_API int kratos_hydro_totals(kratos_hydro_t *h, double out[5]);
+
+/* Number of times a primitive floor (rho, p >= 1e-30) fired since create.  n: host.  Synchronises. */
+KRATOS_API int kratos_hydro_floor_hits(kratos_hydro_t *h, long long *n);
+
+/* Number of kernel launches this handle has issued since create.  n: host.  No synchronisation. */
+KRATOS_API int kratos_hydro_launch_count(kratos_hydro_t *h, long long *n);
+
+/* Per-kernel timing with CUDA events on the handle's stream.  enable != 0 switches event
+ * recording on for step / run; kratos_hydro_get_timing then returns, since the last call to
+ * set_profiling, the summed duration [ms] and launch count of: slot 0 stage-1 kernel,
+ * slot 1 stage-2 kernel, slot 2 all other kernels (dt bookkeeping, reductions).
+ * ms, launches: host arrays of 3.  Synchronises. */
+KRATOS_API int kratos_hydro_set_profiling(kratos_hydro_t *h, int enable);
+KRATOS_API int kratos_hydro_get_timing(kratos_hydro_t *h, double ms[3], long long launches[3]);
+
+/* Message of the last error raised on this thread ("" if none).  Never NULL. */
+KRATOS_API const char *kratos_hydro_last_error(void);
+
+/* Library version string, e.g. "kratos-hydro-b200 0.1 (sm_100a)". */
+KRATOS_API const char *kratos_hydro_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KRATOS_HYDRO_H */

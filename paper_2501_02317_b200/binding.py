@@ -1,0 +1,240 @@
+"""Thin ctypes front end of the C-ABI in ``include/kratos_hydro.h`` -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libkratos_hydro.so``; there is no Python or
+CPU fallback: if the library is missing it is built with nvcc, and if that fails, or no CUDA
+device is present when a solver is created, an exception is raised.
+
+PyTorch is used for device memory and streams only (``torch.Tensor.data_ptr()``,
+``torch.cuda.current_stream().cuda_stream``); numpy arrays are accepted as host buffers.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+PREC_MIXED, PREC_FP64 = 0, 1
+BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED = 0, 1, 2
+OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
+
+# every symbol include/kratos_hydro.h declares
+SYMBOLS = [
+    "kratos_hydro_create", "kratos_hydro_destroy", "kratos_hydro_set_spacing", "kratos_hydro_set_stream",
+    "kratos_hydro_set_kernel", "kratos_hydro_set_zchunk", "kratos_hydro_set_state", "kratos_hydro_get_state",
+    "kratos_hydro_cfl_dt", "kratos_hydro_step", "kratos_hydro_run", "kratos_hydro_run_until",
+    "kratos_hydro_totals", "kratos_hydro_floor_hits", "kratos_hydro_launch_count",
+    "kratos_hydro_set_profiling", "kratos_hydro_get_timing", "kratos_hydro_last_error", "kratos_hydro_version",
+]
+
+_lib = None
+
+
+class KratosError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"kratos_hydro error {code}: {msg}")
+        self.code = code
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load() -> ctypes.CDLL:
+    """Load (building first if needed) the C-ABI library and declare its signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    if not os.path.exists(path):
+        raise ImportError("libkratos_hydro.so is missing and could not be built: no fallback exists")
+    L = ctypes.CDLL(path)
+    vp, d, i = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    dp, ip, llp = ctypes.POINTER(d), ctypes.POINTER(i), ctypes.POINTER(ctypes.c_longlong)
+    L.kratos_hydro_create.restype = vp
+    L.kratos_hydro_create.argtypes = [i, i, i, d, i, ip]
+    L.kratos_hydro_destroy.restype = None
+    L.kratos_hydro_destroy.argtypes = [vp]
+    L.kratos_hydro_set_spacing.restype = i
+    L.kratos_hydro_set_spacing.argtypes = [vp, d, d, d]
+    L.kratos_hydro_set_stream.restype = i
+    L.kratos_hydro_set_stream.argtypes = [vp, vp]
+    L.kratos_hydro_set_kernel.restype = i
+    L.kratos_hydro_set_kernel.argtypes = [vp, i]
+    L.kratos_hydro_set_zchunk.restype = i
+    L.kratos_hydro_set_zchunk.argtypes = [vp, i]
+    L.kratos_hydro_set_state.restype = i
+    L.kratos_hydro_set_state.argtypes = [vp, vp, i]
+    L.kratos_hydro_get_state.restype = i
+    L.kratos_hydro_get_state.argtypes = [vp, vp, i]
+    L.kratos_hydro_cfl_dt.restype = i
+    L.kratos_hydro_cfl_dt.argtypes = [vp, d, dp]
+    L.kratos_hydro_step.restype = i
+    L.kratos_hydro_step.argtypes = [vp, d]
+    L.kratos_hydro_run.restype = i
+    L.kratos_hydro_run.argtypes = [vp, d, i, dp]
+    L.kratos_hydro_run_until.restype = i
+    L.kratos_hydro_run_until.argtypes = [vp, d, d, i, dp, ip]
+    L.kratos_hydro_totals.restype = i
+    L.kratos_hydro_totals.argtypes = [vp, dp]
+    L.kratos_hydro_floor_hits.restype = i
+    L.kratos_hydro_floor_hits.argtypes = [vp, llp]
+    L.kratos_hydro_launch_count.restype = i
+    L.kratos_hydro_launch_count.argtypes = [vp, llp]
+    L.kratos_hydro_set_profiling.restype = i
+    L.kratos_hydro_set_profiling.argtypes = [vp, i]
+    L.kratos_hydro_get_timing.restype = i
+    L.kratos_hydro_get_timing.argtypes = [vp, dp, llp]
+    L.kratos_hydro_last_error.restype = ctypes.c_char_p
+    L.kratos_hydro_last_error.argtypes = []
+    L.kratos_hydro_version.restype = ctypes.c_char_p
+    L.kratos_hydro_version.argtypes = []
+    _lib = L
+    return L
+
+
+def last_error() -> str:
+    return load().kratos_hydro_last_error().decode()
+
+
+def version() -> str:
+    return load().kratos_hydro_version().decode()
+
+
+def _check(rc: int):
+    if rc != OK:
+        raise KratosError(rc, last_error())
+
+
+def _buffer(x):
+    """(address, on_device, keepalive) of a numpy array or torch tensor holding 5*N float64."""
+    if isinstance(x, np.ndarray):
+        if x.dtype != np.float64 or not x.flags.c_contiguous:
+            raise ValueError("host buffer must be C-contiguous float64")
+        return x.ctypes.data, 0, x
+    import torch
+    if isinstance(x, torch.Tensor):
+        if x.dtype != torch.float64 or not x.is_contiguous():
+            raise ValueError("tensor must be contiguous float64")
+        return x.data_ptr(), 1 if x.is_cuda else 0, x
+    raise TypeError(type(x))
+
+
+class KratosHydro:
+    """One uniform block on the current CUDA device.  Method names mirror the C entry points."""
+
+    def __init__(self, nx, ny, nz, gamma, bc, precision=PREC_MIXED, spacing=None, kernel=KERNEL_AUTO,
+                 stream=None):
+        L = load()
+        self._L = L
+        self.shape = (int(nx), int(ny), int(nz))
+        self.ncell = int(nx) * int(ny) * int(nz)
+        bc_arr = (ctypes.c_int * 6)(*[int(b) for b in bc])
+        self._h = L.kratos_hydro_create(int(nx), int(ny), int(nz), float(gamma), int(precision), bc_arr)
+        if not self._h:
+            raise KratosError(ERR_ARG, last_error())
+        if spacing is not None:
+            self.set_spacing(*spacing)
+        if kernel != KERNEL_AUTO:
+            self.set_kernel(kernel)
+        if stream is not None:
+            self.set_stream(stream)
+
+    # -- lifetime
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._L.kratos_hydro_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    # -- configuration
+    def set_spacing(self, dx, dy, dz):
+        _check(self._L.kratos_hydro_set_spacing(self._h, float(dx), float(dy), float(dz)))
+
+    def set_stream(self, stream):
+        """``stream``: a torch.cuda.Stream, a raw cudaStream_t integer, or None/0 for the default stream."""
+        ptr = getattr(stream, "cuda_stream", stream) or 0
+        _check(self._L.kratos_hydro_set_stream(self._h, ctypes.c_void_p(int(ptr))))
+
+    def set_kernel(self, variant):
+        _check(self._L.kratos_hydro_set_kernel(self._h, int(variant)))
+
+    def set_zchunk(self, planes):
+        _check(self._L.kratos_hydro_set_zchunk(self._h, int(planes)))
+
+    # -- state
+    def set_state(self, U):
+        ptr, dev, _keep = _buffer(U)
+        n = U.size if isinstance(U, np.ndarray) else U.numel()
+        if n != 5 * self.ncell:
+            raise ValueError("state must hold 5*nx*ny*nz values")
+        _check(self._L.kratos_hydro_set_state(self._h, ctypes.c_void_p(ptr), dev))
+
+    def get_state(self, out=None):
+        nx, ny, nz = self.shape
+        if out is None:
+            out = np.empty((5, nz, ny, nx), dtype=np.float64)
+        ptr, dev, _keep = _buffer(out)
+        _check(self._L.kratos_hydro_get_state(self._h, ctypes.c_void_p(ptr), dev))
+        return out
+
+    # -- the path
+    def cfl_dt(self, cfl):
+        dt = ctypes.c_double(0.0)
+        _check(self._L.kratos_hydro_cfl_dt(self._h, float(cfl), ctypes.byref(dt)))
+        return dt.value
+
+    def step(self, dt):
+        _check(self._L.kratos_hydro_step(self._h, float(dt)))
+
+    def run(self, cfl, nsteps, t0=0.0):
+        t = ctypes.c_double(float(t0))
+        _check(self._L.kratos_hydro_run(self._h, float(cfl), int(nsteps), ctypes.byref(t)))
+        return t.value
+
+    def run_until(self, cfl, t_end, max_steps=10 ** 7, t0=0.0):
+        t = ctypes.c_double(float(t0))
+        n = ctypes.c_int(0)
+        _check(self._L.kratos_hydro_run_until(self._h, float(cfl), float(t_end), int(max_steps),
+                                              ctypes.byref(t), ctypes.byref(n)))
+        return t.value, n.value
+
+    # -- diagnostics
+    def totals(self):
+        out = (ctypes.c_double * 5)()
+        _check(self._L.kratos_hydro_totals(self._h, out))
+        return np.array(out[:])
+
+    def floor_hits(self):
+        n = ctypes.c_longlong(0)
+        _check(self._L.kratos_hydro_floor_hits(self._h, ctypes.byref(n)))
+        return n.value
+
+    def launch_count(self):
+        n = ctypes.c_longlong(0)
+        _check(self._L.kratos_hydro_launch_count(self._h, ctypes.byref(n)))
+        return n.value
+
+    def set_profiling(self, enable=True):
+        _check(self._L.kratos_hydro_set_profiling(self._h, 1 if enable else 0))
+
+    def get_timing(self):
+        """{'stage1': (ms, launches), 'stage2': ..., 'other': ...} since set_profiling."""
+        ms = (ctypes.c_double * 3)()
+        n = (ctypes.c_longlong * 3)()
+        _check(self._L.kratos_hydro_get_timing(self._h, ms, n))
+        return {k: (ms[i], n[i]) for i, k in enumerate(("stage1", "stage2", "other"))}

@@ -1,0 +1,464 @@
+// kh_api.cu -- the C-ABI of include/kratos_hydro.h: argument checking, memory, launches.
+// No arithmetic of the method lives here; every step of the path runs in the kernels of
+// kh_simple.cuh / kh_tiled.cuh / kh_reduce.cuh.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/kratos_hydro.h"
+#include "kh_device.cuh"
+#include "kh_reduce.cuh"
+#include "kh_simple.cuh"
+#include "kh_tiled.cuh"
+
+using namespace kh;
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                            \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(e_ == cudaErrorMemoryAllocation ? KRATOS_ERR_ALLOC : KRATOS_ERR_CUDA,     \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                                 \
+    } while (0)
+
+enum { SLOT_STAGE1 = 0, SLOT_STAGE2 = 1, SLOT_OTHER = 2 };
+
+struct kratos_hydro {
+    Grid g;
+    int prec;        // KRATOS_PREC_*
+    int variant;     // resolved KRATOS_KERNEL_SIMPLE / _TILED
+    bool tiled_ok;   // tiled kernel supports this block
+    int zchunk;      // 0 = auto
+    double* U0;      // current state (device)
+    double* U1;      // predictor (device)
+    Ctrl* ctrl;      // device
+    Ctrl* h_ctrl;    // pinned host mirror
+    dd* partial;     // totals scratch (device)
+    double* d_tot;   // 5 doubles (device)
+    int tot_blocks;
+    cudaStream_t stream;
+    bool rate_valid;  // ctrl->rate_bits holds the rate maximum of U0
+    long long launches;
+    // profiling
+    bool profiling;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<std::pair<int, int>> ev_used;  // (slot, index of start event; stop = +1)
+    size_t ev_next;
+    double prof_ms[3];
+    long long prof_n[3];
+};
+
+const char* kratos_hydro_last_error(void) { return g_err; }
+const char* kratos_hydro_version(void) { return "kratos-hydro-b200 0.1 (sm_100a)"; }
+
+// ---------------------------------------------------------------------------------------
+namespace {
+
+struct LaunchTimer {
+    kratos_hydro* h;
+    int slot;
+    int idx;
+    LaunchTimer(kratos_hydro* h_, int slot_) : h(h_), slot(slot_), idx(-1)
+    {
+        h->launches++;
+        if (!h->profiling) return;
+        if (h->ev_next + 2 > h->ev_pool.size()) {
+            if (h->ev_pool.size() >= 200000) return;  // stop recording, keep running
+            for (int i = 0; i < 2; i++) {
+                cudaEvent_t e;
+                if (cudaEventCreate(&e) != cudaSuccess) return;
+                h->ev_pool.push_back(e);
+            }
+        }
+        idx = (int)h->ev_next;
+        h->ev_next += 2;
+        cudaEventRecord(h->ev_pool[idx], h->stream);
+    }
+    ~LaunchTimer()
+    {
+        if (idx < 0) return;
+        cudaEventRecord(h->ev_pool[idx + 1], h->stream);
+        h->ev_used.push_back({slot, idx});
+    }
+};
+
+void collect_timing(kratos_hydro* h)
+{
+    for (auto& u : h->ev_used) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->ev_pool[u.second], h->ev_pool[u.second + 1]) == cudaSuccess) {
+            h->prof_ms[u.first] += ms;
+            h->prof_n[u.first] += 1;
+        }
+    }
+    h->ev_used.clear();
+    h->ev_next = 0;
+}
+
+int pick_zchunk(const kratos_hydro* h)
+{
+    if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
+    return tiled_auto_zchunk(h->g);
+}
+
+template <typename T>
+int launch_stage(kratos_hydro* h, int stage)
+{
+    const Grid& g = h->g;
+    const double* Uin = (stage == 1) ? h->U0 : h->U1;
+    double* Uout = (stage == 1) ? h->U1 : h->U0;
+    LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
+    if (h->variant == KRATOS_KERNEL_TILED) {
+        launch_stage_tiled<T>(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
+    } else {
+        const int threads = 128;
+        const long long blocks = (g.N + threads - 1) / threads;
+        if (stage == 1)
+            stage_simple<T, 1><<<(unsigned)blocks, threads, 0, h->stream>>>(Uin, h->U0, Uout, g, h->ctrl);
+        else
+            stage_simple<T, 2><<<(unsigned)blocks, threads, 0, h->stream>>>(Uin, h->U0, Uout, g, h->ctrl);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "stage %d launch: %s", stage, cudaGetErrorString(e));
+    return KRATOS_OK;
+}
+
+int launch_both_stages(kratos_hydro* h)
+{
+    int rc;
+    if (h->prec == KRATOS_PREC_MIXED) {
+        if ((rc = launch_stage<float>(h, 1))) return rc;
+        return launch_stage<float>(h, 2);
+    }
+    if ((rc = launch_stage<double>(h, 1))) return rc;
+    return launch_stage<double>(h, 2);
+}
+
+int launch_cfl_rate(kratos_hydro* h)
+{
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        reset_rate_kernel<<<1, 1, 0, h->stream>>>(h->ctrl);
+    }
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        long long blocks = (h->g.N + 255) / 256;
+        if (blocks > 148 * 8) blocks = 148 * 8;
+        cfl_rate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "cfl launch: %s", cudaGetErrorString(e));
+    h->rate_valid = true;
+    return KRATOS_OK;
+}
+
+__global__ void configure_run_kernel(Ctrl* ctrl, double cfl, double t_end, double t)
+{
+    ctrl->cfl = cfl;
+    ctrl->t_end = t_end;
+    ctrl->t = t;
+    ctrl->steps = 0;
+    ctrl->nonfinite = 0;
+}
+
+int read_ctrl(kratos_hydro* h)
+{
+    CUDA_TRY(cudaMemcpyAsync(h->h_ctrl, h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return KRATOS_OK;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------
+kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int scheme, const int bc[6])
+{
+    g_err[0] = 0;
+    const int n[3] = {nx, ny, nz};
+    if (!bc) { fail(KRATOS_ERR_ARG, "bc is NULL"); return nullptr; }
+    if (!(gamma > 1.0) || !std::isfinite(gamma)) { fail(KRATOS_ERR_ARG, "gamma must be > 1"); return nullptr; }
+    const int prec = scheme & 3, integ = (scheme >> 4) & 3;
+    if ((prec != KRATOS_PREC_MIXED && prec != KRATOS_PREC_FP64) || integ != 0 || (scheme & ~0x33)) {
+        fail(KRATOS_ERR_ARG, "unsupported scheme word 0x%x", scheme);
+        return nullptr;
+    }
+    int nactive = 0;
+    for (int d = 0; d < 3; d++) {
+        if (n[d] < 1 || (n[d] > 1 && n[d] < 4)) {
+            fail(KRATOS_ERR_ARG, "extent %d of axis %d: active axes need >= 4 cells", n[d], d);
+            return nullptr;
+        }
+        if (n[d] > 1) {
+            nactive++;
+            const int lo = bc[2 * d], hi = bc[2 * d + 1];
+            if (lo < 0 || lo > 3 || hi < 0 || hi > 3) { fail(KRATOS_ERR_ARG, "bad bc code on axis %d", d); return nullptr; }
+            if ((lo == KRATOS_BC_PERIODIC) != (hi == KRATOS_BC_PERIODIC)) {
+                fail(KRATOS_ERR_ARG, "periodic on one side only of axis %d", d);
+                return nullptr;
+            }
+        }
+    }
+    if (nactive == 0) { fail(KRATOS_ERR_ARG, "no active axis"); return nullptr; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        fail(KRATOS_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+        return nullptr;
+    }
+    kratos_hydro* h = new (std::nothrow) kratos_hydro();
+    if (!h) { fail(KRATOS_ERR_ALLOC, "host allocation failed"); return nullptr; }
+    Grid& g = h->g;
+    g.N = 1;
+    for (int d = 0; d < 3; d++) {
+        g.n[d] = n[d];
+        g.active[d] = n[d] > 1;
+        g.bc[2 * d] = g.active[d] ? bc[2 * d] : 0;
+        g.bc[2 * d + 1] = g.active[d] ? bc[2 * d + 1] : 0;
+        g.inv_dx[d] = g.active[d] ? (double)n[d] : 0.0;
+        g.N *= n[d];
+    }
+    g.gamma = gamma;
+    h->prec = prec;
+    h->tiled_ok = g.active[0] && g.active[1];
+    h->variant = h->tiled_ok ? KRATOS_KERNEL_TILED : KRATOS_KERNEL_SIMPLE;
+    h->zchunk = 0;
+    h->stream = 0;
+    h->rate_valid = false;
+    h->launches = 0;
+    h->profiling = false;
+    h->ev_next = 0;
+    for (int s = 0; s < 3; s++) { h->prof_ms[s] = 0; h->prof_n[s] = 0; }
+    h->U0 = h->U1 = nullptr;
+    h->ctrl = nullptr; h->h_ctrl = nullptr; h->partial = nullptr; h->d_tot = nullptr;
+    h->tot_blocks = (int)((g.N + 255) / 256 < 592 ? (g.N + 255) / 256 : 592);
+    const size_t bytes = sizeof(double) * 5 * (size_t)g.N;
+    cudaError_t e;
+    if ((e = cudaMalloc(&h->U0, bytes)) != cudaSuccess || (e = cudaMalloc(&h->U1, bytes)) != cudaSuccess ||
+        (e = cudaMalloc(&h->ctrl, sizeof(Ctrl))) != cudaSuccess ||
+        (e = cudaMalloc(&h->partial, sizeof(dd) * 5 * h->tot_blocks)) != cudaSuccess ||
+        (e = cudaMalloc(&h->d_tot, sizeof(double) * 5)) != cudaSuccess ||
+        (e = cudaMallocHost(&h->h_ctrl, sizeof(Ctrl) + 64)) != cudaSuccess ||
+        (e = cudaMemset(h->ctrl, 0, sizeof(Ctrl))) != cudaSuccess ||
+        (e = cudaMemset(h->U0, 0, bytes)) != cudaSuccess || (e = cudaMemset(h->U1, 0, bytes)) != cudaSuccess) {
+        fail(e == cudaErrorMemoryAllocation ? KRATOS_ERR_ALLOC : KRATOS_ERR_CUDA, "create: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        kratos_hydro_destroy(h);
+        return nullptr;
+    }
+    tiled_configure();
+    return h;
+}
+
+void kratos_hydro_destroy(kratos_hydro_t* h)
+{
+    if (!h) return;
+    cudaFree(h->U0);
+    cudaFree(h->U1);
+    cudaFree(h->ctrl);
+    cudaFree(h->partial);
+    cudaFree(h->d_tot);
+    if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
+    for (auto e : h->ev_pool) cudaEventDestroy(e);
+    delete h;
+}
+
+int kratos_hydro_set_spacing(kratos_hydro_t* h, double dx, double dy, double dz)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    const double s[3] = {dx, dy, dz};
+    for (int d = 0; d < 3; d++)
+        if (h->g.active[d] && (!(s[d] > 0.0) || !std::isfinite(s[d]))) return fail(KRATOS_ERR_ARG, "spacing must be > 0");
+    for (int d = 0; d < 3; d++) h->g.inv_dx[d] = h->g.active[d] ? 1.0 / s[d] : 0.0;
+    h->rate_valid = false;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_stream(kratos_hydro_t* h, void* cuda_stream)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    h->stream = (cudaStream_t)cuda_stream;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    if (variant == KRATOS_KERNEL_AUTO) variant = h->tiled_ok ? KRATOS_KERNEL_TILED : KRATOS_KERNEL_SIMPLE;
+    if (variant == KRATOS_KERNEL_TILED && !h->tiled_ok)
+        return fail(KRATOS_ERR_ARG, "tiled kernel needs active x and y axes");
+    if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED) return fail(KRATOS_ERR_ARG, "bad variant");
+    h->variant = variant;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_zchunk(kratos_hydro_t* h, int planes)
+{
+    if (!h || planes < 0) return fail(KRATOS_ERR_ARG, "bad argument");
+    h->zchunk = planes;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_state(kratos_hydro_t* h, const double* U, int on_device)
+{
+    if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
+    const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
+    CUDA_TRY(cudaMemcpyAsync(h->U0, U, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->rate_valid = false;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_get_state(kratos_hydro_t* h, double* U, int on_device)
+{
+    if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
+    const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
+    CUDA_TRY(cudaMemcpyAsync(U, h->U0, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return KRATOS_OK;
+}
+
+int kratos_hydro_cfl_dt(kratos_hydro_t* h, double cfl, double* dt_out)
+{
+    if (!h || !dt_out) return fail(KRATOS_ERR_ARG, "NULL argument");
+    if (!(cfl > 0.0) || !std::isfinite(cfl)) return fail(KRATOS_ERR_ARG, "cfl must be > 0");
+    int rc;
+    if ((rc = launch_cfl_rate(h))) return rc;
+    if ((rc = read_ctrl(h))) return rc;
+    double rate;
+    memcpy(&rate, &h->h_ctrl->rate_bits, sizeof(double));
+    const double dt = cfl / rate;
+    *dt_out = dt;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(KRATOS_ERR_NONFINITE, "non-finite CFL time step (rate %g)", rate);
+    return KRATOS_OK;
+}
+
+int kratos_hydro_step(kratos_hydro_t* h, double dt)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(KRATOS_ERR_ARG, "dt must be > 0 and finite");
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        set_dt_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, dt);
+    }
+    int rc = launch_both_stages(h);
+    if (rc) return rc;
+    h->rate_valid = true;  // stage 2 left the rate maximum of the new state in ctrl
+    return KRATOS_OK;
+}
+
+static int run_impl(kratos_hydro_t* h, double cfl, double t_end, int max_steps, double* t_inout, int* steps_done)
+{
+    if (!h || !t_inout) return fail(KRATOS_ERR_ARG, "NULL argument");
+    if (!(cfl > 0.0) || !std::isfinite(cfl) || max_steps < 0) return fail(KRATOS_ERR_ARG, "bad cfl / step count");
+    if (!std::isfinite(*t_inout) || !std::isfinite(t_end)) return fail(KRATOS_ERR_ARG, "non-finite time");
+    int rc;
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        configure_run_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, cfl, t_end > 0.0 ? t_end : 0.0, *t_inout);
+    }
+    if (!h->rate_valid && (rc = launch_cfl_rate(h))) return rc;
+    int done = 0;
+    const int batch = (t_end > 0.0) ? 64 : max_steps;
+    while (done < max_steps) {
+        const int nb = (max_steps - done < batch) ? max_steps - done : batch;
+        for (int s = 0; s < nb; s++) {
+            {
+                LaunchTimer lt(h, SLOT_OTHER);
+                prepare_step_kernel<<<1, 1, 0, h->stream>>>(h->ctrl);
+            }
+            if ((rc = launch_both_stages(h))) return rc;
+        }
+        done += nb;
+        if ((rc = read_ctrl(h))) return rc;
+        if (h->h_ctrl->nonfinite) break;
+        if (t_end > 0.0 && h->h_ctrl->t >= t_end) break;
+    }
+    if (done == 0 && (rc = read_ctrl(h))) return rc;
+    *t_inout = h->h_ctrl->t;
+    if (steps_done) *steps_done = (int)h->h_ctrl->steps;
+    h->rate_valid = !h->h_ctrl->nonfinite;
+    if (h->h_ctrl->nonfinite) return fail(KRATOS_ERR_NONFINITE, "non-finite time step during run (t = %g)", h->h_ctrl->t);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "run: %s", cudaGetErrorString(e));
+    return KRATOS_OK;
+}
+
+int kratos_hydro_run(kratos_hydro_t* h, double cfl, int nsteps, double* t_inout)
+{
+    return run_impl(h, cfl, 0.0, nsteps, t_inout, nullptr);
+}
+
+int kratos_hydro_run_until(kratos_hydro_t* h, double cfl, double t_end, int max_steps, double* t_inout, int* steps_done)
+{
+    if (!(t_end > 0.0)) return fail(KRATOS_ERR_ARG, "t_end must be > 0");
+    return run_impl(h, cfl, t_end, max_steps, t_inout, steps_done);
+}
+
+int kratos_hydro_totals(kratos_hydro_t* h, double out[5])
+{
+    if (!h || !out) return fail(KRATOS_ERR_ARG, "NULL argument");
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        totals_kernel<<<dim3(h->tot_blocks, 5), 256, 0, h->stream>>>(h->U0, h->g.N, h->partial);
+    }
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        totals_final_kernel<<<1, 32, 0, h->stream>>>(h->partial, h->tot_blocks, h->d_tot);
+    }
+    double* scratch = reinterpret_cast<double*>(reinterpret_cast<char*>(h->h_ctrl) + sizeof(Ctrl));
+    static_assert(sizeof(Ctrl) % 8 == 0, "Ctrl must keep doubles aligned");
+    CUDA_TRY(cudaMemcpyAsync(scratch, h->d_tot, sizeof(double) * 5, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (int m = 0; m < 5; m++) out[m] = scratch[m];
+    return KRATOS_OK;
+}
+
+int kratos_hydro_floor_hits(kratos_hydro_t* h, long long* n)
+{
+    if (!h || !n) return fail(KRATOS_ERR_ARG, "NULL argument");
+    int rc = read_ctrl(h);
+    if (rc) return rc;
+    *n = (long long)h->h_ctrl->floor_hits;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_launch_count(kratos_hydro_t* h, long long* n)
+{
+    if (!h || !n) return fail(KRATOS_ERR_ARG, "NULL argument");
+    *n = h->launches;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_profiling(kratos_hydro_t* h, int enable)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->ev_used.clear();
+    h->ev_next = 0;
+    for (int s = 0; s < 3; s++) { h->prof_ms[s] = 0; h->prof_n[s] = 0; }
+    h->profiling = enable != 0;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_get_timing(kratos_hydro_t* h, double ms[3], long long launches[3])
+{
+    if (!h || !ms || !launches) return fail(KRATOS_ERR_ARG, "NULL argument");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    collect_timing(h);
+    for (int s = 0; s < 3; s++) { ms[s] = h->prof_ms[s]; launches[s] = h->prof_n[s]; }
+    return KRATOS_OK;
+}

@@ -1,0 +1,116 @@
+// kh_reduce.cuh -- reductions and time-step bookkeeping kernels.
+#pragma once
+#include "kh_device.cuh"
+
+namespace kh {
+
+// CFL rate maximum of the stored state, fp64 in every precision mode (S1, S7).
+// Grid-stride, warp-shuffle + one atomicMax per block.
+__global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict__ U, Grid g, Ctrl* ctrl)
+{
+    __shared__ double red[32];
+    double rate = 0.0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < g.N;
+         c += (long long)gridDim.x * blockDim.x) {
+        const double u[5] = {U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c]};
+        double r = cfl_rate_from_cons<double>(u, g);
+        if (!(r == r)) r = __longlong_as_double(0x7ff0000000000000LL);
+        rate = fmax(rate, r);
+    }
+    block_atomic_max_nonneg(rate, &ctrl->rate_bits, red);
+}
+
+// dt bookkeeping between steps of kratos_hydro_run: one thread.
+//   dt = cfl / rate_max, clipped to land on t_end; t += dt; reset the reduction target.
+__global__ void prepare_step_kernel(Ctrl* ctrl)
+{
+    const double rate = __longlong_as_double((long long)ctrl->rate_bits);
+    double dt = ctrl->cfl / rate;
+    if (!(dt > 0.0) || !(dt < __longlong_as_double(0x7ff0000000000000LL))) {
+        ctrl->nonfinite = 1;
+        dt = 0.0;
+    }
+    if (ctrl->t_end > 0.0) {
+        const double left = ctrl->t_end - ctrl->t;
+        if (left <= 0.0) dt = 0.0;
+        else if (ctrl->t + dt >= ctrl->t_end) dt = left;
+    }
+    ctrl->dt = dt;
+    if (dt > 0.0) {
+        // landing exactly: t + (t_end - t) may differ from t_end in the last bit
+        const double tn = ctrl->t + dt;
+        ctrl->t = (ctrl->t_end > 0.0 && dt == ctrl->t_end - ctrl->t) ? ctrl->t_end : tn;
+        ctrl->steps += 1;
+        ctrl->rate_bits = 0ull;  // stage 2 of this step reduces the next rate
+    }
+}
+
+// kratos_hydro_step(dt): the caller's dt.
+__global__ void set_dt_kernel(Ctrl* ctrl, double dt)
+{
+    ctrl->dt = dt;
+    ctrl->t += dt;
+    ctrl->rate_bits = 0ull;
+}
+
+__global__ void reset_rate_kernel(Ctrl* ctrl) { ctrl->rate_bits = 0ull; }
+
+// ---------------------------------------------------------------------------------------
+// double-double accumulation (error-free transformations) for the conservation diagnostics.
+struct dd {
+    double hi, lo;
+};
+__device__ __forceinline__ dd dd_add(dd a, double b)
+{
+    const double s = a.hi + b;
+    const double bb = s - a.hi;
+    const double e = (a.hi - (s - bb)) + (b - bb);  // TwoSum
+    const double lo = a.lo + e;
+    const double hi = s + lo;
+    return dd{hi, lo - (hi - s)};
+}
+__device__ __forceinline__ dd dd_add(dd a, dd b)
+{
+    const double s = a.hi + b.hi;
+    const double bb = s - a.hi;
+    const double e = (a.hi - (s - bb)) + (b.hi - bb);
+    const double lo = (a.lo + b.lo) + e;
+    const double hi = s + lo;
+    return dd{hi, lo - (hi - s)};
+}
+
+// partial[field][block] = double-double sum of that block's share.  Launch with 256 threads.
+__global__ void __launch_bounds__(256) totals_kernel(const double* __restrict__ U, long long N, dd* partial)
+{
+    __shared__ dd red[8];
+    const int field = blockIdx.y;
+    const double* f = U + (long long)field * N;
+    dd acc{0.0, 0.0};
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < N;
+         c += (long long)gridDim.x * blockDim.x)
+        acc = dd_add(acc, f[c]);
+    for (int o = 16; o > 0; o >>= 1) {
+        dd other{__shfl_xor_sync(0xffffffffu, acc.hi, o), __shfl_xor_sync(0xffffffffu, acc.lo, o)};
+        acc = dd_add(acc, other);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) red[warp] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        dd t = red[0];
+        for (int w = 1; w < 8; w++) t = dd_add(t, red[w]);
+        partial[(long long)field * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// out[field] = sum over blocks, one thread per field.
+__global__ void totals_final_kernel(const dd* partial, int nblocks, double* out)
+{
+    const int field = threadIdx.x;
+    if (field >= 5) return;
+    dd t{0.0, 0.0};
+    for (int b = 0; b < nblocks; b++) t = dd_add(t, partial[(long long)field * nblocks + b]);
+    out[field] = t.hi + t.lo;
+}
+
+}  // namespace kh

@@ -1,0 +1,296 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 CPU oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json's: relative L1 per conserved field
+<= 1e-12 in all-fp64 mode, <= 1e-5 in mixed precision; conserved totals drift <= 1e-13.
+
+Run with  python -m pytest tests -m gpu  on a B200 box.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2501_02317_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+P, F, O, R = 0, 1, 2, 3
+MIXED, FP64 = binding.PREC_MIXED, binding.PREC_FP64
+SIMPLE, TILED = binding.KERNEL_SIMPLE, binding.KERNEL_TILED
+TOL = {MIXED: 1e-5, FP64: 1e-12}
+
+
+def rel_l1_fields(got, ref):
+    """Per-field relative L1; fields identically zero in the oracle must be identically zero."""
+    out = []
+    for m in range(5):
+        den = np.abs(ref[m]).sum()
+        if den == 0.0:
+            assert np.all(got[m] == 0.0), f"field {m} must stay exactly zero"
+            out.append(0.0)
+        else:
+            out.append(float(np.abs(got[m] - ref[m]).sum() / den))
+    return out
+
+
+def make(pr, prec, kernel=binding.KERNEL_AUTO):
+    nx, ny, nz = pr.shape
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, kernel=kernel)
+    h.set_state(pr.U)
+    return h
+
+
+def lockstep(pr, prec, kernel, nsteps, cfl=0.4):
+    """Both sides take the oracle's dt sequence (an input like any other); returns (gpu, oracle)."""
+    Uo = pr.U.copy()
+    h = make(pr, prec, kernel)
+    for _ in range(nsteps):
+        dt = oracle.cfl_dt(Uo, pr.gamma, cfl)
+        oracle.step(Uo, pr.gamma, pr.bc, dt)
+        h.step(dt)
+    Ug = h.get_state()
+    hits = h.floor_hits()
+    h.destroy()
+    return Ug, Uo, hits
+
+
+# --------------------------------------------------------------------------- basics
+def test_state_roundtrip_and_totals():
+    pr = inputs.random_smooth(37, 21, 9, seed=1)
+    h = make(pr, MIXED)
+    np.testing.assert_array_equal(h.get_state(), pr.U)
+    tot = h.totals()
+    exact = np.array([math.fsum(pr.U[m].ravel()) for m in range(5)])
+    np.testing.assert_allclose(tot, exact, rtol=2e-16, atol=1e-300)
+    # device-resident buffers through torch
+    import torch
+    Ud = torch.from_numpy(pr.U).cuda()
+    h.set_state(Ud * 2.0)
+    out = torch.empty_like(Ud)
+    h.get_state(out)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(out.cpu().numpy(), pr.U * 2.0)
+    h.destroy()
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 50), (1, 40, 1), (33, 1, 1), (1, 24, 36), (20, 1, 17), (9, 21, 37)])
+def test_cfl_dt_matches_oracle(shape):
+    nz, ny, nx = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=2)
+    for prec in (MIXED, FP64):
+        h = make(pr, prec)
+        assert h.cfl_dt(0.4) == pytest.approx(oracle.cfl_dt(pr.U, pr.gamma, 0.4), rel=1e-13)
+        h.destroy()
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+def test_uniform_state_is_bitwise_fixed_point(prec, kernel):
+    U0 = inputs.prim_to_cons(np.full((12, 20, 40), 1.3), 0.7, 0.4, -1.1, 2.2, 1.4)
+    for bc in ((P,) * 6, (F,) * 6):
+        pr = inputs.Problem("uniform", np.ascontiguousarray(U0), 1.4, bc)
+        h = make(pr, prec, kernel)
+        for _ in range(3):
+            h.step(1e-3)
+        np.testing.assert_array_equal(h.get_state(), U0)
+        h.destroy()
+
+
+# --------------------------------------------------------------------------- element-wise parity, small ragged cases
+CASES_3D = [
+    ((45, 19, 23), (P, P, P, P, P, P)),
+    ((37, 33, 10), (F, F, O, O, R, R)),
+    ((32, 16, 8), (R, O, P, P, F, R)),
+    ((70, 35, 5), (O, R, F, O, P, P)),
+]
+CASES_2D = [((37, 21, 1), (P, P, P, P, P, P)), ((64, 48, 1), (R, R, O, F, P, P)), ((33, 5, 1), (F, O, R, R, P, P))]
+CASES_ANY = [((50, 1, 1), (F, F, P, P, P, P)), ((1, 40, 1), (P, P, R, O, P, P)), ((1, 1, 33), (P, P, P, P, O, R)),
+             ((24, 1, 18), (P, P, P, P, F, F)), ((1, 20, 22), (P, P, R, R, P, P))]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+@pytest.mark.parametrize("shape,bc", CASES_3D + CASES_2D)
+def test_parity_small_ragged(shape, bc, kernel, prec):
+    nx, ny, nz = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=nx + ny + nz, gamma=1.4, bc=bc)
+    Ug, Uo, hits = lockstep(pr, prec, kernel, 5)
+    assert hits == 0
+    err = rel_l1_fields(Ug, Uo)
+    assert max(err) <= TOL[prec], err
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("shape,bc", CASES_ANY)
+def test_parity_other_axis_combinations(shape, bc, prec):
+    """1D along y or z, x-z and y-z planes: served by the general (simple) kernel."""
+    nx, ny, nz = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=5, gamma=5.0 / 3.0, bc=bc)
+    Ug, Uo, hits = lockstep(pr, prec, binding.KERNEL_AUTO, 6)
+    assert hits == 0
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("zchunk", [4, 7, 16, 1000])
+def test_slab_seams_do_not_change_the_result(zchunk):
+    """Marching slabs of different height must give bit-identical states (one flux per face)."""
+    pr = inputs.random_smooth(40, 20, 29, seed=8, gamma=1.4)
+    ref = None
+    for zc in (zchunk, 29):
+        h = make(pr, MIXED, TILED)
+        h.set_zchunk(zc)
+        for _ in range(3):
+            h.step(2e-3)
+        U = h.get_state()
+        h.destroy()
+        if ref is None:
+            ref = U
+        else:
+            np.testing.assert_array_equal(U, ref)
+
+
+def test_strong_jumps_take_every_hllc_branch():
+    rng = np.random.default_rng(9)
+    nz, ny, nx = 12, 18, 40
+    rho = rng.uniform(0.1, 2.0, (nz, ny, nx))
+    p = rng.uniform(0.05, 2.0, (nz, ny, nx))
+    v = rng.uniform(-2.5, 2.5, (3, nz, ny, nx))
+    U = np.ascontiguousarray(inputs.prim_to_cons(rho, p, v[0], v[1], v[2], 1.4))
+    pr = inputs.Problem("jumps", U, 1.4, (P,) * 6)
+    L, hits = oracle.flux_divergence(U, 1.4, pr.bc)
+    assert hits == 0
+    dt = 1e-4
+    for kernel in (SIMPLE, TILED):
+        for prec in (MIXED, FP64):
+            h = make(pr, prec, kernel)
+            h.step(dt)
+            Ug = h.get_state()
+            h.destroy()
+            Uo = U.copy()
+            oracle.step(Uo, 1.4, pr.bc, dt)
+            # compare the increments: dU/dt against the oracle's
+            num = np.abs((Ug - U) - (Uo - U)).sum(axis=(1, 2, 3))
+            den = np.abs(Uo - U).sum(axis=(1, 2, 3))
+            assert (num / den).max() <= (3e-6 if prec == MIXED else 1e-11)
+
+
+# --------------------------------------------------------------------------- configs (reduced twins)
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_c1_riemann_1d(seed, axis, prec):
+    """C1: 256 cells, gamma 1.4, Free BC, cfl 0.4, t = 0.2 -- self-driven run on both sides."""
+    if axis != 0 and seed > 2:
+        pytest.skip("axis interchange covered with two seeds")
+    pr = inputs.riemann_1d(seed, 256, axis=axis)
+    Uo = pr.U.copy()
+    to, no, _ = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.2)
+    h = make(pr, prec)
+    tg, ng = h.run_until(0.4, 0.2)
+    Ug = h.get_state()
+    assert h.floor_hits() == 0
+    h.destroy()
+    assert tg == pytest.approx(0.2, abs=1e-15)
+    assert abs(ng - no) <= (0 if prec == FP64 else 1)
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c2_advected_wave_reduced(prec):
+    pr = inputs.advected_wave_2d(64, t_end=0.5)
+    Uo = pr.U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.5)
+    h = make(pr, prec)
+    tg, _ = h.run_until(0.4, 0.5)
+    Ug = h.get_state()
+    h.destroy()
+    assert tg == 0.5
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c3_shear_layer_reduced(prec):
+    pr = inputs.shear_layer_2d(256, seed=3, nsteps=100)
+    Uo = pr.U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 100)
+    h = make(pr, prec)
+    h.run(0.4, 100)
+    Ug = h.get_state()
+    h.destroy()
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c4_point_blast_reduced(prec):
+    pr = inputs.point_blast_3d(64, nsteps=50)
+    Uo = pr.U.copy()
+    _, _, hits_o = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 50)
+    h = make(pr, prec)
+    h.run(0.4, 50)
+    Ug = h.get_state()
+    hits = h.floor_hits()
+    h.destroy()
+    assert hits == 0 and hits_o == 0
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c5_turbulence_reduced(prec):
+    pr = inputs.turbulence_3d(64, seed=5, nsteps=20)
+    Uo = pr.U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 20)
+    h = make(pr, prec)
+    h.run(0.4, 20)
+    Ug = h.get_state()
+    h.destroy()
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+
+
+# --------------------------------------------------------------------------- conservation (P3) on the GPU
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+def test_periodic_conservation(prec, kernel):
+    pr = inputs.turbulence_3d(48, seed=7, nsteps=30)
+    h = make(pr, prec, kernel)
+    T0 = h.totals()
+    A0 = np.array([math.fsum(np.abs(pr.U[m]).ravel()) for m in range(5)])
+    h.run(0.4, 30)
+    T1 = h.totals()
+    U = h.get_state()
+    h.destroy()
+    np.testing.assert_allclose(T1, [math.fsum(U[m].ravel()) for m in range(5)], rtol=2e-16, atol=1e-18 * A0.max())
+    drift = np.abs(T1 - T0) / np.maximum(np.abs(T0), A0)
+    assert drift.max() <= 1e-13, drift
+
+
+def test_run_equals_manual_stepping_in_fp64():
+    """run() (device-resident dt) and cfl_dt()+step() give the same bits in all-fp64 mode."""
+    pr = inputs.random_smooth(40, 24, 12, seed=4)
+    h1 = make(pr, FP64)
+    t1 = h1.run(0.4, 6)
+    h2 = make(pr, FP64)
+    t2 = 0.0
+    for _ in range(6):
+        dt = h2.cfl_dt(0.4)
+        h2.step(dt)
+        t2 += dt
+    np.testing.assert_array_equal(h1.get_state(), h2.get_state())
+    assert t1 == pytest.approx(t2, rel=1e-15)
+    h1.destroy()
+    h2.destroy()
+
+
+def test_step_rejects_bad_dt_and_nonfinite_state_is_reported():
+    pr = inputs.random_smooth(32, 16, 1, seed=4)
+    h = make(pr, MIXED)
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(binding.KratosError) as ei:
+            h.step(bad)
+        assert ei.value.code == binding.ERR_ARG
+    U = pr.U.copy()
+    U[0, 0, 3, 3] = float("nan")
+    h.set_state(U)
+    with pytest.raises(binding.KratosError) as ei:
+        h.cfl_dt(0.4)
+    assert ei.value.code == binding.ERR_NONFINITE
+    h.destroy()
