@@ -36,6 +36,7 @@ static int fail(int code, const char* fmt, ...)
     } while (0)
 
 enum { SLOT_STAGE1 = 0, SLOT_STAGE2 = 1, SLOT_OTHER = 2 };
+enum { CFL_MAX_BLOCKS = 148 * 8 };
 
 struct kratos_hydro {
     Grid g;
@@ -49,6 +50,7 @@ struct kratos_hydro {
     Ctrl* h_ctrl;    // pinned host mirror
     dd* partial;     // totals scratch (device)
     double* d_tot;   // 5 doubles (device)
+    double* p_partial;  // per-block pressure sums of the cfl kernel (device)
     int tot_blocks;
     cudaStream_t stream;
     bool rate_valid;  // ctrl->rate_bits holds the rate maximum of U0
@@ -157,8 +159,10 @@ int launch_cfl_rate(kratos_hydro* h)
     {
         LaunchTimer lt(h, SLOT_OTHER);
         long long blocks = (h->g.N + 255) / 256;
-        if (blocks > 148 * 8) blocks = 148 * 8;
-        cfl_rate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl);
+        if (blocks > CFL_MAX_BLOCKS) blocks = CFL_MAX_BLOCKS;
+        cfl_rate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl, h->p_partial);
+        finish_cfl_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, h->p_partial, (int)blocks, 1.0 / (double)h->g.N);
+        h->launches++;
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "cfl launch: %s", cudaGetErrorString(e));
@@ -243,7 +247,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->ev_next = 0;
     for (int s = 0; s < 3; s++) { h->prof_ms[s] = 0; h->prof_n[s] = 0; }
     h->U0 = h->U1 = nullptr;
-    h->ctrl = nullptr; h->h_ctrl = nullptr; h->partial = nullptr; h->d_tot = nullptr;
+    h->ctrl = nullptr; h->h_ctrl = nullptr; h->partial = nullptr; h->d_tot = nullptr; h->p_partial = nullptr;
     h->tot_blocks = (int)((g.N + 255) / 256 < 592 ? (g.N + 255) / 256 : 592);
     const size_t bytes = sizeof(double) * 5 * (size_t)g.N;
     cudaError_t e;
@@ -251,6 +255,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         (e = cudaMalloc(&h->ctrl, sizeof(Ctrl))) != cudaSuccess ||
         (e = cudaMalloc(&h->partial, sizeof(dd) * 5 * h->tot_blocks)) != cudaSuccess ||
         (e = cudaMalloc(&h->d_tot, sizeof(double) * 5)) != cudaSuccess ||
+        (e = cudaMalloc(&h->p_partial, sizeof(double) * CFL_MAX_BLOCKS)) != cudaSuccess ||
         (e = cudaMallocHost(&h->h_ctrl, sizeof(Ctrl) + 64)) != cudaSuccess ||
         (e = cudaMemset(h->ctrl, 0, sizeof(Ctrl))) != cudaSuccess ||
         (e = cudaMemset(h->U0, 0, bytes)) != cudaSuccess || (e = cudaMemset(h->U1, 0, bytes)) != cudaSuccess) {
@@ -271,6 +276,7 @@ void kratos_hydro_destroy(kratos_hydro_t* h)
     cudaFree(h->ctrl);
     cudaFree(h->partial);
     cudaFree(h->d_tot);
+    cudaFree(h->p_partial);
     if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
     for (auto e : h->ev_pool) cudaEventDestroy(e);
     delete h;

@@ -27,6 +27,7 @@ struct Ctrl {
     unsigned long long rate_bits;    // max over cells of sum_d (|v_d|+c)/dx_d, as double bits (>= 0)
     unsigned long long floor_hits;   // primitive floor activations (reading S6)
     long long steps;                 // steps with dt > 0 taken by run / run_until
+    double p_ref;                    // reference pressure of the mixed-precision momentum flux (fp32-exact)
     int nonfinite;                   // set when a dt came out non-finite
     int pad;
 };
@@ -102,8 +103,20 @@ __device__ __forceinline__ float rsqrt_(float x)
 }
 __device__ __forceinline__ double rsqrt_(double x) { return 1.0 / sqrt(x); }
 
+// Explicitly rounded arithmetic: the compiler neither contracts nor re-associates these, so every
+// inlined copy of the flux and slope functions computes bit-identical results from identical inputs
+// (a face shared by two tiles or two slabs is evaluated by two thread blocks).
+__device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_(float a, float b) { return __fadd_rn(a, -b); }
+__device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub_(double a, double b) { return __dadd_rn(a, -b); }
+__device__ __forceinline__ double mul_(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+
 // c = sqrt(gamma p / rho).  fp32: gamma p * rsqrt(gamma p rho), a single MUFU.
-__device__ __forceinline__ float sound_speed(float gp, float rho) { return gp * rsqrt_(gp * rho); }
+__device__ __forceinline__ float sound_speed(float gp, float rho) { return mul_(gp, rsqrt_(mul_(gp, rho))); }
 __device__ __forceinline__ double sound_speed(double gp, double rho) { return sqrt(gp / rho); }
 
 // ---------------------------------------------------------------------------------------
@@ -136,12 +149,19 @@ __device__ __forceinline__ int cons_to_prim(double rho, double mx, double my, do
     return hits;
 }
 
-// Eq. 3, reading S2 for ab = 0.
-template <typename T>
-__device__ __forceinline__ T minmod(T a, T b)
+// Eq. 3, reading S2 for ab = 0: the argument of smaller magnitude when both have
+// the same sign, else 0.  fp32: FMNMX.XORSIGN gives min(|a|,|b|) carrying sign(a) xor sign(b); clamping
+// at 0 keeps it only for equal signs; the sign of a is put back with one LOP3 -- three ALU instructions.
+__device__ __forceinline__ float minmod(float a, float b)
 {
-    const T m = fmin(fabs(a), fabs(b));
-    return (a * b > T(0)) ? copysign(m, a) : T(0);
+    float t;
+    asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(t) : "f"(a), "f"(b));
+    return copysignf(fmaxf(t, 0.0f), a);
+}
+__device__ __forceinline__ double minmod(double a, double b)
+{
+    const double m = fmin(fabs(a), fabs(b));
+    return ((a > 0.0) == (b > 0.0) && a != 0.0 && b != 0.0) ? copysign(m, a) : 0.0;
 }
 
 // Half the limited undivided difference: (dx/2) * minmod((q0-qm)/dx, (qp-q0)/dx) on a uniform
@@ -150,7 +170,7 @@ __device__ __forceinline__ T minmod(T a, T b)
 template <typename T>
 __device__ __forceinline__ T half_slope(T qm, T q0, T qp)
 {
-    return T(0.5) * minmod(q0 - qm, qp - q0);
+    return mul_(T(0.5), minmod(sub_(q0, qm), sub_(qp, q0)));  // the product with 1/2 is exact
 }
 
 // Constants of the Riemann solver, computed once per kernel.
@@ -159,8 +179,9 @@ struct GasConst {
     T gamma;   // gamma
     T g1;      // (gamma+1)/(2 gamma), Eq. 5
     T igm1;    // 1/(gamma-1)
-    __device__ __forceinline__ explicit GasConst(double g)
-        : gamma(T(g)), g1(T((g + 1.0) / (2.0 * g))), igm1(T(1.0 / (g - 1.0))) {}
+    T pref;    // reference pressure: face states carry p - pref (0 in all-fp64 mode)
+    __device__ __forceinline__ GasConst(double g, double p_ref)
+        : gamma(T(g)), g1(T((g + 1.0) / (2.0 * g))), igm1(T(1.0 / (g - 1.0))), pref(T(p_ref)) {}
 };
 
 // Sec. 3.2.2: HLLC flux with the subtraction-safe wave speeds of Eq. 5.
@@ -168,60 +189,69 @@ struct GasConst {
 //   p_* = max(0, (p_L+p_R)/2 - (u_R-u_L)/2 * rho_bar * c_bar)                        (reading S3)
 //   q_K = sqrt(1 + (gamma+1)/(2 gamma) * max(p_*/p_K - 1, 0)),  Delta s_L = -c_L q_L,  Delta s_R = +c_R q_R
 //   s_* = {[p_R - rho_R u_R Ds_R] - [p_L - rho_L u_L Ds_L]} / {rho_L Ds_L - rho_R Ds_R}        (Eq. 4)
-// Flux on the side K of the contact that contains x/t = 0, written in Ds_K throughout
+// Selection in the standard order: s_L >= 0: F_L; else s_* >= 0: F*_L; else s_R > 0: F*_R; else F_R
+// (with the acoustic p_* estimate s_L <= s_* is not guaranteed for strong compressions, so the order
+// of the tests is part of the definition).  Flux on the selected side K, written in Ds_K throughout
 // (an algebraically equivalent form of the star-state assembly, reading S4):
 //   m_K = rho_K Ds_K,  p_*K = p_K + m_K (s_* - u_K),  phi = s_* / (s_K - s_*),
 //   F_rho = phi m_K,  F_u = p_*K + F_rho s_*,  F_E = s_* [ (E_K Ds_K - p_K u_K)/(s_K - s_*) + p_*K (1 + phi) ],
-//   F_v = F_rho v_K,  F_w = F_rho w_K;
-// outside the fan (s_L >= 0 or s_R <= 0) the upwind physical flux.
-// F = (mass, normal momentum, tangential momentum 1, tangential momentum 2, energy).
+//   F_v = F_rho v_K,  F_w = F_rho w_K;   outside the fan the upwind physical flux.
+//
+// Pressure enters as the deviation p' = p - pref (L.p, R.p hold p'): in the same spirit as Eq. 5, the
+// momentum flux is formed without the large common term -- F_u returned here is F_u - pref, which has
+// the same face-to-face differences on a uniform mesh, so that nearly uniform pressure does not cost
+// the fp32 flux difference its significant digits.  With pref = 0 this is the plain form.
+// F = (mass, normal momentum - pref, tangential momentum 1, tangential momentum 2, energy).
 template <typename T>
 __device__ __forceinline__ void hllc(const Prim<T>& L, const Prim<T>& R, const GasConst<T>& gc, T F[5])
 {
-    const T cL = sound_speed(gc.gamma * L.p, L.r);
-    const T cR = sound_speed(gc.gamma * R.p, R.r);
+    const T pL = add_(L.p, gc.pref), pR = add_(R.p, gc.pref);  // actual pressures
+    const T cL = sound_speed(mul_(gc.gamma, pL), L.r);
+    const T cR = sound_speed(mul_(gc.gamma, pR), R.r);
 
-    T pst = T(0.5) * (L.p + R.p) - T(0.125) * (R.u - L.u) * (L.r + R.r) * (cL + cR);
-    pst = fmax(pst, T(0));
+    // p_* as a deviation from pref, clipped so that the actual value is >= 0
+    const T w = mul_(mul_(sub_(R.u, L.u), add_(L.r, R.r)), add_(cL, cR));
+    T pst = fma_(T(-0.125), w, mul_(T(0.5), add_(L.p, R.p)));
+    pst = fmax(pst, -gc.pref);
 
-    const T qL = sqrt_(T(1) + gc.g1 * fmax(pst * rcp_(L.p) - T(1), T(0)));
-    const T qR = sqrt_(T(1) + gc.g1 * fmax(pst * rcp_(R.p) - T(1), T(0)));
-    const T dsL = -cL * qL;
-    const T dsR = cR * qR;
-    const T mL = L.r * dsL;
-    const T mR = R.r * dsR;
-    const T sst = ((R.p - mR * R.u) - (L.p - mL * L.u)) * rcp_(mL - mR);
+    const T qL = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, L.p), rcp_(pL)), T(0)), T(1)));
+    const T qR = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, R.p), rcp_(pR)), T(0)), T(1)));
+    const T dsL = -mul_(cL, qL);
+    const T dsR = mul_(cR, qR);
+    const T mL = mul_(L.r, dsL);
+    const T mR = mul_(R.r, dsR);
+    const T sst = mul_(sub_(fma_(-mR, R.u, R.p), fma_(-mL, L.u, L.p)), rcp_(sub_(mL, mR)));
 
-    // selection in the standard order: s_L >= 0: F_L;  else s_* >= 0: F*_L;  else s_R > 0: F*_R;  else F_R.
-    // (With the acoustic p_* estimate s_L <= s_* is not guaranteed for strong compressions, so the
-    //  order of the tests is part of the definition.)
-    const bool left = (L.u + dsL >= T(0)) || (sst >= T(0));
+    const bool left = (add_(L.u, dsL) >= T(0)) || (sst >= T(0));
     const T rK = left ? L.r : R.r;
-    const T pK = left ? L.p : R.p;
+    const T pKd = left ? L.p : R.p;
     const T uK = left ? L.u : R.u;
     const T vK = left ? L.v : R.v;
     const T wK = left ? L.w : R.w;
     const T dsK = left ? dsL : dsR;
     const T mK = left ? mL : mR;
-    const T sK = uK + dsK;
-    const bool outer = left ? (sK >= T(0)) : !(sK > T(0));
+    const T pK = add_(pKd, gc.pref);
+    const T sK = add_(uK, dsK);
+    const bool outer = (left ? sK : -sK) >= T(0);  // s_L >= 0, resp. s_R <= 0
 
-    const T EK = pK * gc.igm1 + T(0.5) * rK * (uK * uK + vK * vK + wK * wK);
-    const T inv = rcp_(sK - sst);
-    const T phi = sst * inv;
-    const T pstK = pK + mK * (sst - uK);
-    T F0 = phi * mK;
-    T F1 = pstK + F0 * sst;
-    T F4 = sst * ((EK * dsK - pK * uK) * inv + pstK * (T(1) + phi));
+    const T ke = fma_(wK, wK, fma_(vK, vK, mul_(uK, uK)));
+    const T EK = fma_(pK, gc.igm1, mul_(mul_(T(0.5), rK), ke));
+    const T inv = rcp_(sub_(sK, sst));
+    const T phi = mul_(sst, inv);
+    const T pstKd = fma_(mK, sub_(sst, uK), pKd);
+    T F0 = mul_(phi, mK);
+    T F1 = fma_(F0, sst, pstKd);
+    const T A4 = fma_(EK, dsK, -mul_(pK, uK));
+    T F4 = mul_(sst, fma_(A4, inv, mul_(add_(pstKd, gc.pref), add_(T(1), phi))));
     if (outer) {
-        F0 = rK * uK;
-        F1 = F0 * uK + pK;
-        F4 = (EK + pK) * uK;
+        F0 = mul_(rK, uK);
+        F1 = fma_(F0, uK, pKd);
+        F4 = mul_(add_(EK, pK), uK);
     }
     F[0] = F0;
     F[1] = F1;
-    F[2] = F0 * vK;
-    F[3] = F0 * wK;
+    F[2] = mul_(F0, vK);
+    F[3] = mul_(F0, wK);
     F[4] = F4;
 }
 
@@ -239,7 +269,7 @@ __device__ __forceinline__ T cfl_rate(T rho, T p, T vx, T vy, T vz, T gamma, T i
 // during the variable conversion, whose output is float_t; fp64 in all-fp64 mode).
 // Used by the standalone cfl kernel (T = double) and by the stage-2 epilogues.
 template <typename T>
-__device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const Grid& g)
+__device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const Grid& g, T* p_out = nullptr)
 {
     T r = T(Un[0]);
     r = (r < T(KH_RHO_FLOOR)) ? T(KH_RHO_FLOOR) : r;  // comparisons, not fmax: a NaN must survive
@@ -247,6 +277,7 @@ __device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const Grid& 
     const T vx = T(Un[1]) * ir, vy = T(Un[2]) * ir, vz = T(Un[3]) * ir;
     T p = T(g.gamma - 1.0) * (T(Un[4]) - T(0.5) * r * (vx * vx + vy * vy + vz * vz));
     p = (p < T(KH_P_FLOOR)) ? T(KH_P_FLOOR) : p;
+    if (p_out) *p_out = p;
     return cfl_rate<T>(r, p, vx, vy, vz, T(g.gamma), T(g.inv_dx[0]), T(g.inv_dx[1]), T(g.inv_dx[2]));
 }
 

@@ -5,19 +5,41 @@
 namespace kh {
 
 // CFL rate maximum of the stored state, fp64 in every precision mode (S1, S7).
-// Grid-stride, warp-shuffle + one atomicMax per block.
-__global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict__ U, Grid g, Ctrl* ctrl)
+// Grid-stride, warp-shuffle + one atomicMax per block.  Also leaves each block's pressure sum in
+// p_partial[blockIdx.x] (fixed reduction order => run-to-run reproducible reference pressure).
+__global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict__ U, Grid g, Ctrl* ctrl,
+                                                       double* p_partial)
 {
     __shared__ double red[32];
-    double rate = 0.0;
+    __shared__ double psum[8];
+    double rate = 0.0, ps = 0.0;
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < g.N;
          c += (long long)gridDim.x * blockDim.x) {
         const double u[5] = {U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c]};
-        double r = cfl_rate_from_cons<double>(u, g);
+        double p;
+        double r = cfl_rate_from_cons<double>(u, g, &p);
         if (!(r == r)) r = __longlong_as_double(0x7ff0000000000000LL);
         rate = fmax(rate, r);
+        ps += p;
     }
-    block_atomic_max_nonneg(rate, &ctrl->rate_bits, red);
+    for (int o = 16; o > 0; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
+    if ((threadIdx.x & 31) == 0) psum[threadIdx.x >> 5] = ps;
+    block_atomic_max_nonneg(rate, &ctrl->rate_bits, red);  // contains a __syncthreads()
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; w++) t += psum[w];
+        p_partial[blockIdx.x] = t;
+    }
+}
+
+// Reference pressure of the mixed-precision momentum flux: the mean pressure, rounded to fp32 so that
+// the fp64 primitive recovery and the fp32 Riemann solver use the very same number.
+__global__ void finish_cfl_kernel(Ctrl* ctrl, const double* p_partial, int nblocks, double inv_n)
+{
+    double t = 0.0;
+    for (int b = 0; b < nblocks; b++) t += p_partial[b];
+    const float m = (float)(t * inv_n);
+    ctrl->p_ref = (m == m && m > 0.0f && m < 3.0e38f) ? (double)m : 0.0;
 }
 
 // dt bookkeeping between steps of kratos_hydro_run: one thread.

@@ -47,7 +47,7 @@ __device__ __noinline__ void face_flux_global(const double* __restrict__ U, cons
                                               int d, T Fout[5])
 {
     const double gm1 = g.gamma - 1.0;
-    const GasConst<T> gc(g.gamma);
+    const GasConst<T> gc(g.gamma, 0.0);
     int c[3] = {ci, cj, ck};
     Prim<T> W[4];
 #pragma unroll
