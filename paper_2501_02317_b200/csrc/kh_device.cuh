@@ -220,9 +220,11 @@ __device__ __forceinline__ void hllc(const Prim<T>& L, const Prim<T>& R, const G
     const T dsR = mul_(cR, qR);
     const T mL = mul_(L.r, dsL);
     const T mR = mul_(R.r, dsR);
-    const T sst = mul_(sub_(fma_(-mR, R.u, R.p), fma_(-mL, L.u, L.p)), rcp_(sub_(mL, mR)));
-
-    const bool left = (add_(L.u, dsL) >= T(0)) || (sst >= T(0));
+    // s_* = num/den (Eq. 4) with den = m_L - m_R < 0, and 1/(s_K - s_*) = den/D with D = s_K den - num:
+    // both quotients from ONE reciprocal, r = 1/(den D).  The side is chosen from signs alone.
+    const T num = sub_(fma_(-mR, R.u, R.p), fma_(-mL, L.u, L.p));
+    const T den = sub_(mL, mR);
+    const bool left = (add_(L.u, dsL) >= T(0)) || (num <= T(0));  // s_L >= 0 or s_* >= 0
     const T rK = left ? L.r : R.r;
     const T pKd = left ? L.p : R.p;
     const T uK = left ? L.u : R.u;
@@ -234,9 +236,12 @@ __device__ __forceinline__ void hllc(const Prim<T>& L, const Prim<T>& R, const G
     const T sK = add_(uK, dsK);
     const bool outer = (left ? sK : -sK) >= T(0);  // s_L >= 0, resp. s_R <= 0
 
+    const T D = fma_(sK, den, -num);
+    const T r = rcp_(mul_(den, D));
+    const T sst = mul_(num, mul_(D, r));
+    const T inv = mul_(den, mul_(den, r));
     const T ke = fma_(wK, wK, fma_(vK, vK, mul_(uK, uK)));
     const T EK = fma_(pK, gc.igm1, mul_(mul_(T(0.5), rK), ke));
-    const T inv = rcp_(sub_(sK, sst));
     const T phi = mul_(sst, inv);
     const T pstKd = fma_(mK, sub_(sst, uK), pKd);
     T F0 = mul_(phi, mK);
@@ -269,16 +274,52 @@ __device__ __forceinline__ T cfl_rate(T rho, T p, T vx, T vy, T vz, T gamma, T i
 // during the variable conversion, whose output is float_t; fp64 in all-fp64 mode).
 // Used by the standalone cfl kernel (T = double) and by the stage-2 epilogues.
 template <typename T>
-__device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const Grid& g, T* p_out = nullptr)
+struct CflConst {
+    T gm1, gamma, idx, idy, idz;
+    __device__ __forceinline__ explicit CflConst(const Grid& g)
+        : gm1(T(g.gamma - 1.0)), gamma(T(g.gamma)), idx(T(g.inv_dx[0])), idy(T(g.inv_dx[1])), idz(T(g.inv_dx[2])) {}
+};
+
+template <typename T>
+__device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const CflConst<T>& cc, T* p_out = nullptr)
 {
     T r = T(Un[0]);
     r = (r < T(KH_RHO_FLOOR)) ? T(KH_RHO_FLOOR) : r;  // comparisons, not fmax: a NaN must survive
     const T ir = rcp_(r);
     const T vx = T(Un[1]) * ir, vy = T(Un[2]) * ir, vz = T(Un[3]) * ir;
-    T p = T(g.gamma - 1.0) * (T(Un[4]) - T(0.5) * r * (vx * vx + vy * vy + vz * vz));
+    T p = cc.gm1 * (T(Un[4]) - T(0.5) * r * (vx * vx + vy * vy + vz * vz));
     p = (p < T(KH_P_FLOOR)) ? T(KH_P_FLOOR) : p;
     if (p_out) *p_out = p;
-    return cfl_rate<T>(r, p, vx, vy, vz, T(g.gamma), T(g.inv_dx[0]), T(g.inv_dx[1]), T(g.inv_dx[2]));
+    return cfl_rate<T>(r, p, vx, vy, vz, cc.gamma, cc.idx, cc.idy, cc.idz);
+}
+
+// ---------------------------------------------------------------------------------------
+// Split-phase block barrier on an mbarrier in shared memory: arrive (release), do independent work,
+// then wait (acquire).  All threads of the block take part in every phase.
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ unsigned long long mbar_arrive(unsigned long long* bar)
+{
+    unsigned long long token;
+    asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];"
+                 : "=l"(token)
+                 : "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+    return token;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned long long token)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        ::"r"((unsigned)__cvta_generic_to_shared(bar)), "l"(token)
+        : "memory");
 }
 
 // ---------------------------------------------------------------------------------------

@@ -13,11 +13,12 @@ __global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict_
     __shared__ double red[32];
     __shared__ double psum[8];
     double rate = 0.0, ps = 0.0;
+    const CflConst<double> cc(g);
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < g.N;
          c += (long long)gridDim.x * blockDim.x) {
         const double u[5] = {U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c]};
         double p;
-        double r = cfl_rate_from_cons<double>(u, g, &p);
+        double r = cfl_rate_from_cons<double>(u, cc, &p);
         if (!(r == r)) r = __longlong_as_double(0x7ff0000000000000LL);
         rate = fmax(rate, r);
         ps += p;

@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(128) stage_simple(const double* __restrict__ U
             Uout[m * g.N + c] = Un[m];
         }
         if (STAGE == 2) {
-            rate = (double)cfl_rate_from_cons<T>(Un, g);
+            rate = (double)cfl_rate_from_cons<T>(Un, CflConst<T>(g));
             if (!(rate == rate)) rate = __longlong_as_double(0x7ff0000000000000LL);
         }
     }

@@ -35,10 +35,16 @@ constexpr int TX = 32;
 // Tile height and resident blocks per SM.  Two independent blocks per SM (mixed precision) keep the
 // pipes busy across each other's barriers: while one block converts fluxes (XU pipe) the other solves
 // Riemann problems (FMA/ALU pipes).
+#ifndef KH_TY_F32
+#define KH_TY_F32 16  // tile height, mixed precision
+#endif
+#ifndef KH_BPS_F32
+#define KH_BPS_F32 1  // resident blocks per SM, mixed precision
+#endif
 template <typename T>
 struct TileShape {
-    static constexpr int TY = 8;
-    static constexpr int BLOCKS_PER_SM = (sizeof(T) == 4) ? 2 : 1;
+    static constexpr int TY = (sizeof(T) == 4) ? KH_TY_F32 : 8;
+    static constexpr int BLOCKS_PER_SM = (sizeof(T) == 4) ? KH_BPS_F32 : 1;
 };
 
 // roles of the warps (one warp per tile row; TY >= 8)
@@ -61,6 +67,7 @@ struct TileSmem {
     T Fx[5][TY][TX + 1];                                   // x-face fluxes, conserved-field order
     T Fy[5][TY + 1][TX];                                   // y-face fluxes
     double red[32];
+    unsigned long long mbar;                               // split-phase barrier between flux and update phases
 };
 
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src)
@@ -150,6 +157,7 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
     const int kend = (NDIM == 3) ? min(kbeg + zchunk, nz) : 1;
     const double gm1 = g.gamma - 1.0;
     const GasConst<T> gc(g.gamma, pref_d);
+    const CflConst<T> cc(g);
     const long long N = g.N;
     const long long pl = (long long)nx * ny;
 
@@ -351,7 +359,7 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
             out[f * N] = Un[f];
         }
         if (STAGE == 2) {
-            T r = cfl_rate_from_cons<T>(Un, g);
+            T r = cfl_rate_from_cons<T>(Un, cc);
             if (!(r == r)) r = T(__int_as_float(0x7f800000));
             rate = fmax(rate, r);
         }
@@ -397,7 +405,9 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
                 Fxlo[f] = Fylo[f] = T(0);
             }
         }
-        // iteration k: fill(k+1) | barrier | flux(k), slopes(k+1), z face k+1/2 | barrier | update(k).
+        if (tx == 0 && ty == 0) mbar_init(&sm.mbar, TX * TY);
+        __syncthreads();
+        // iteration k: fill(k+1) | barrier | flux(k), slopes(k+1) | arrive | z face k+1/2 | wait | update(k).
         // k = kbeg-1 only primes the pipeline (tile and slopes of plane kbeg, low z face of the slab).
 #pragma unroll 1
         for (int k = kbeg - 1; k < kend; k++) {
@@ -412,6 +422,8 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
             __syncthreads();
             if (k >= kbeg) fluxes(k, W0, hsx, hsy);
             if (next) slopes(k + 1, Wp1, hsx, hsy);
+            // arrive now, wait after the z face: that work needs nothing from other threads
+            const unsigned long long token = mbar_arrive(&sm.mbar);
             // z face k+1/2 from the register-resident column
             convert_own(k + 2, Wp2, k + 2 < kend);
             T hs1[5];
@@ -429,7 +441,7 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
                 for (int f = 0; f < 5; f++) Fzhi[f] = (double)F[f];
             }
             if (STAGE == 2) __pipeline_wait_prior(1);  // U0(k) has landed (own thread's copy)
-            __syncthreads();
+            mbar_wait(&sm.mbar, token);                // every thread's x/y fluxes of plane k are published
             if (k >= kbeg) update_cell(k, Fzlo, Fzhi);
             if (k + 1 < kend) fetch_u0(k + 1);  // single slot: only after this thread has read U0(k)
             __pipeline_commit();
@@ -452,9 +464,9 @@ inline int tiled_auto_zchunk(const Grid& g)
 {
     if (!g.active[2]) return 1;
     // enough thread blocks for >= ~12 waves over 148 SMs (one block per SM), slabs of >= 16 planes
-    const long long tiles = (long long)((g.n[0] + TX - 1) / TX) * ((g.n[1] + 7) / 8);
+    const long long tiles = (long long)((g.n[0] + TX - 1) / TX) * ((g.n[1] + KH_TY_F32 - 1) / KH_TY_F32);
     int chunk = g.n[2];
-    while (chunk > 16 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * 2 * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 16 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * KH_BPS_F32 * 12) chunk = (chunk + 1) / 2;
     return chunk;
 }
 
@@ -465,6 +477,8 @@ inline void tiled_set_attr()
     static_assert(sizeof(S) * TileShape<T>::BLOCKS_PER_SM <= 227 * 1024 - 1024 * TileShape<T>::BLOCKS_PER_SM,
                   "tiles do not fit the shared memory of one SM");
     cudaFuncSetAttribute(stage_tiled<T, STAGE, NDIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(S));
+    cudaFuncSetAttribute(stage_tiled<T, STAGE, NDIM>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                         (int)cudaSharedmemCarveoutMaxShared);
 }
 
 inline void tiled_configure()
