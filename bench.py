@@ -50,6 +50,11 @@ def workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
+def kernel_name(prec: int, stage: int, ndim: int) -> str:
+    """Name of the stage kernel the library launches for this block."""
+    return f"stage_tiled<{'float' if prec == 0 else 'double'},{stage},{ndim}>"
+
+
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -59,14 +64,19 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(workload_name: str, precision: str):
-    """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this workload."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+def ncu_traffic(workload_name: str, precision: str, kernel: str):
+    """DRAM bytes per launch (read + write) of `kernel` from the committed ncu --set full capture
+    (profiles/traffic.csv, written from the capture named in its `source` column), or None."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path) as f:
-            return json.load(f).get(f"{workload_name}:{precision}")
+            for row in csv.DictReader(f):
+                if row["workload"] == workload_name and row["precision"] == precision and row["kernel"] == kernel:
+                    return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -255,10 +265,10 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
-        roofline = {"bound": "hbm", "kernel": f"stage_tiled<{'float' if prec == 0 else 'double'},{dom[-1]},3>"
-                    if nz > 1 else f"stage_tiled<...,{dom[-1]},2>",
-                    "achieved": kern[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                    "frac": kern[dom]["frac"], "traffic": ncu_traffic(args.workload, args.precision),
+        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2)
+        roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
+                    "unit": "GB/s", "frac": kern[dom]["frac"],
+                    "traffic": ncu_traffic(args.workload, args.precision, kname),
                     "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL[dom]}
     step_frac = value / world * 200.0 / (peak * 1e9)
 
