@@ -52,7 +52,7 @@ def workload(name: str):
 
 def kernel_name(prec: int, stage: int, ndim: int) -> str:
     """Name of the stage kernel the library launches for this block."""
-    return f"stage_tiled<{'float' if prec == 0 else 'double'},{stage},{ndim}>"
+    return f"stage_pair<{stage},{ndim}>" if prec == 0 else f"stage_tiled<double,{stage},{ndim}>"
 
 
 def measured_peak():

@@ -13,6 +13,7 @@
 #include "kh_reduce.cuh"
 #include "kh_simple.cuh"
 #include "kh_tiled.cuh"
+#include "kh_pair.cuh"
 
 using namespace kh;
 
@@ -111,10 +112,16 @@ void collect_timing(kratos_hydro* h)
     h->ev_next = 0;
 }
 
+int auto_variant(const kratos_hydro* h)
+{
+    if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
+    return h->prec == KRATOS_PREC_MIXED ? KRATOS_KERNEL_PAIRED : KRATOS_KERNEL_TILED;
+}
+
 int pick_zchunk(const kratos_hydro* h)
 {
     if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
-    return tiled_auto_zchunk(h->g);
+    return h->variant == KRATOS_KERNEL_PAIRED ? pr::auto_zchunk(h->g) : tiled_auto_zchunk(h->g);
 }
 
 template <typename T>
@@ -124,7 +131,9 @@ int launch_stage(kratos_hydro* h, int stage)
     const double* Uin = (stage == 1) ? h->U0 : h->U1;
     double* Uout = (stage == 1) ? h->U1 : h->U0;
     LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
-    if (h->variant == KRATOS_KERNEL_TILED) {
+    if (h->variant == KRATOS_KERNEL_PAIRED) {
+        pr::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
+    } else if (h->variant == KRATOS_KERNEL_TILED) {
         launch_stage_tiled<T>(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else {
         const int threads = 128;
@@ -217,6 +226,10 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         }
     }
     if (nactive == 0) { fail(KRATOS_ERR_ARG, "no active axis"); return nullptr; }
+    if ((long long)nx * ny >= (1LL << 31) || (long long)nx * ny * nz >= (1LL << 40)) {
+        fail(KRATOS_ERR_ARG, "block too large: nx*ny must be < 2^31 cells");
+        return nullptr;
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -238,7 +251,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     g.gamma = gamma;
     h->prec = prec;
     h->tiled_ok = g.active[0] && g.active[1];
-    h->variant = h->tiled_ok ? KRATOS_KERNEL_TILED : KRATOS_KERNEL_SIMPLE;
+    h->variant = auto_variant(h);
     h->zchunk = 0;
     h->stream = 0;
     h->rate_valid = false;
@@ -265,6 +278,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         return nullptr;
     }
     tiled_configure();
+    pr::configure();
     return h;
 }
 
@@ -303,10 +317,13 @@ int kratos_hydro_set_stream(kratos_hydro_t* h, void* cuda_stream)
 int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
-    if (variant == KRATOS_KERNEL_AUTO) variant = h->tiled_ok ? KRATOS_KERNEL_TILED : KRATOS_KERNEL_SIMPLE;
-    if (variant == KRATOS_KERNEL_TILED && !h->tiled_ok)
-        return fail(KRATOS_ERR_ARG, "tiled kernel needs active x and y axes");
-    if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED) return fail(KRATOS_ERR_ARG, "bad variant");
+    if (variant == KRATOS_KERNEL_AUTO) variant = auto_variant(h);
+    if ((variant == KRATOS_KERNEL_TILED || variant == KRATOS_KERNEL_PAIRED) && !h->tiled_ok)
+        return fail(KRATOS_ERR_ARG, "tiled and paired kernels need active x and y axes");
+    if (variant == KRATOS_KERNEL_PAIRED && h->prec != KRATOS_PREC_MIXED)
+        return fail(KRATOS_ERR_ARG, "the paired kernel is the mixed-precision path");
+    if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED && variant != KRATOS_KERNEL_PAIRED)
+        return fail(KRATOS_ERR_ARG, "bad variant");
     h->variant = variant;
     return KRATOS_OK;
 }

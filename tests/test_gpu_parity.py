@@ -16,7 +16,8 @@ pytestmark = pytest.mark.gpu
 
 P, F, O, R = 0, 1, 2, 3
 MIXED, FP64 = binding.PREC_MIXED, binding.PREC_FP64
-SIMPLE, TILED = binding.KERNEL_SIMPLE, binding.KERNEL_TILED
+SIMPLE, TILED, PAIRED = binding.KERNEL_SIMPLE, binding.KERNEL_TILED, binding.KERNEL_PAIRED
+KERNELS = [SIMPLE, TILED, PAIRED]
 TOL = {MIXED: 1e-5, FP64: 1e-12}
 
 
@@ -34,6 +35,8 @@ def rel_l1_fields(got, ref):
 
 
 def make(pr, prec, kernel=binding.KERNEL_AUTO):
+    if kernel == PAIRED and prec != MIXED:
+        pytest.skip("the paired kernel is the mixed-precision path")
     nx, ny, nz = pr.shape
     h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, kernel=kernel)
     h.set_state(pr.U)
@@ -84,7 +87,7 @@ def test_cfl_dt_matches_oracle(shape):
 
 
 @pytest.mark.parametrize("prec", [MIXED, FP64])
-@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+@pytest.mark.parametrize("kernel", KERNELS)
 def test_uniform_state_is_bitwise_fixed_point(prec, kernel):
     U0 = inputs.prim_to_cons(np.full((12, 20, 40), 1.3), 0.7, 0.4, -1.1, 2.2, 1.4)
     for bc in ((P,) * 6, (F,) * 6):
@@ -109,7 +112,7 @@ CASES_ANY = [((50, 1, 1), (F, F, P, P, P, P)), ((1, 40, 1), (P, P, R, O, P, P)),
 
 
 @pytest.mark.parametrize("prec", [MIXED, FP64])
-@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("shape,bc", CASES_3D + CASES_2D)
 def test_parity_small_ragged(shape, bc, kernel, prec):
     nx, ny, nz = shape
@@ -131,13 +134,14 @@ def test_parity_other_axis_combinations(shape, bc, prec):
     assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
 
 
+@pytest.mark.parametrize("kernel", [TILED, PAIRED])
 @pytest.mark.parametrize("zchunk", [4, 7, 16, 1000])
-def test_slab_seams_do_not_change_the_result(zchunk):
+def test_slab_seams_do_not_change_the_result(zchunk, kernel):
     """Marching slabs of different height must give bit-identical states (one flux per face)."""
     pr = inputs.random_smooth(40, 20, 29, seed=8, gamma=1.4)
     ref = None
     for zc in (zchunk, 29):
-        h = make(pr, MIXED, TILED)
+        h = make(pr, MIXED, kernel)
         h.set_zchunk(zc)
         for _ in range(3):
             h.step(2e-3)
@@ -160,8 +164,10 @@ def test_strong_jumps_take_every_hllc_branch():
     L, hits = oracle.flux_divergence(U, 1.4, pr.bc)
     assert hits == 0
     dt = 1e-4
-    for kernel in (SIMPLE, TILED):
+    for kernel in KERNELS:
         for prec in (MIXED, FP64):
+            if kernel == PAIRED and prec != MIXED:
+                continue
             h = make(pr, prec, kernel)
             h.step(dt)
             Ug = h.get_state()
@@ -248,7 +254,7 @@ def test_c5_turbulence_reduced(prec):
 
 # --------------------------------------------------------------------------- conservation (P3) on the GPU
 @pytest.mark.parametrize("prec", [MIXED, FP64])
-@pytest.mark.parametrize("kernel", [SIMPLE, TILED])
+@pytest.mark.parametrize("kernel", KERNELS)
 def test_periodic_conservation(prec, kernel):
     pr = inputs.turbulence_3d(48, seed=7, nsteps=30)
     h = make(pr, prec, kernel)
