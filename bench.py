@@ -50,9 +50,15 @@ def workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
-def kernel_name(prec: int, stage: int, ndim: int) -> str:
+def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto") -> str:
     """Name of the stage kernel the library launches for this block."""
-    return f"stage_pair<{stage},{ndim}>" if prec == 0 else f"stage_tiled<double,{stage},{ndim}>"
+    if variant == "simple":
+        return f"stage_simple<{'float' if prec == 0 else 'double'},{stage}>"
+    if prec == 0 and (variant == "roles" or (variant == "auto" and ndim == 3)):
+        return f"stage_roles<{stage}>"
+    if prec == 0 and variant in ("auto", "paired"):
+        return f"stage_pair<{stage},{ndim}>"
+    return f"stage_tiled<{'float' if prec == 0 else 'double'},{stage},{ndim}>"
 
 
 def measured_peak():
@@ -72,7 +78,8 @@ def ncu_traffic(workload_name: str, precision: str, kernel: str):
     try:
         with open(path) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload_name and row["precision"] == precision and row["kernel"] == kernel:
+                if (row["workload"] == workload_name and row["precision"] == precision
+                        and kernel.replace(" ", "") in row["kernel"].replace(" ", "")):
                     return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
     except Exception:
         pass
@@ -186,7 +193,11 @@ def run_ours(args):
     nx, ny, nz = pr.shape
     ncell = pr.ncell
     stream = torch.cuda.Stream()
-    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream)
+    variant = {"auto": binding.KERNEL_AUTO, "simple": binding.KERNEL_SIMPLE, "tiled": binding.KERNEL_TILED,
+               "paired": binding.KERNEL_PAIRED, "roles": binding.KERNEL_ROLES}[args.kernel]
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream, kernel=variant)
+    if args.zchunk > 0:
+        h.set_zchunk(args.zchunk)
     host = torch.from_numpy(pr.U).pin_memory()            # pinned host copy (e2e leg)
     with torch.cuda.stream(stream):
         dev = host.to("cuda", non_blocking=True)
@@ -265,7 +276,7 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
-        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2)
+        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel)
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                     "unit": "GB/s", "frac": kern[dom]["frac"],
                     "traffic": ncu_traffic(args.workload, args.precision, kname),
@@ -286,7 +297,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32 flux / f64 state" if prec == 0 else "f64", "data": "synthetic",
         "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": args.precision,
-                   "scheme": "PLM-minmod + HLLC + Heun", "cfl": pr.cfl, "parallelism": f"replicas x{world}",
+                   "scheme": "PLM-minmod + HLLC + Heun", "kernel": args.kernel, "cfl": pr.cfl, "parallelism": f"replicas x{world}",
                    "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
                    if 40 * ncell > 2.5e8 else "state fits L2: no flush between steps (steps are data-dependent)",
                    "floor_hits": hits},
@@ -311,6 +322,9 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "roles"],
+                    help="stage kernel variant (default: the library's own choice)")
+    ap.add_argument("--zchunk", type=int, default=0, help="planes per slab of the marching kernels (0 = auto)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -14,6 +14,7 @@
 #include "kh_simple.cuh"
 #include "kh_tiled.cuh"
 #include "kh_pair.cuh"
+#include "kh_role.cuh"
 
 using namespace kh;
 
@@ -115,13 +116,15 @@ void collect_timing(kratos_hydro* h)
 int auto_variant(const kratos_hydro* h)
 {
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
-    return h->prec == KRATOS_PREC_MIXED ? KRATOS_KERNEL_PAIRED : KRATOS_KERNEL_TILED;
+    if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
+    return h->g.active[2] ? KRATOS_KERNEL_ROLES : KRATOS_KERNEL_PAIRED;
 }
 
 int pick_zchunk(const kratos_hydro* h)
 {
     if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
-    return h->variant == KRATOS_KERNEL_PAIRED ? pr::auto_zchunk(h->g) : tiled_auto_zchunk(h->g);
+    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES) ? pr::auto_zchunk(h->g)
+                                                                                      : tiled_auto_zchunk(h->g);
 }
 
 template <typename T>
@@ -131,7 +134,9 @@ int launch_stage(kratos_hydro* h, int stage)
     const double* Uin = (stage == 1) ? h->U0 : h->U1;
     double* Uout = (stage == 1) ? h->U1 : h->U0;
     LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
-    if (h->variant == KRATOS_KERNEL_PAIRED) {
+    if (h->variant == KRATOS_KERNEL_ROLES) {
+        rl::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
+    } else if (h->variant == KRATOS_KERNEL_PAIRED) {
         pr::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_TILED) {
         launch_stage_tiled<T>(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
@@ -279,6 +284,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     }
     tiled_configure();
     pr::configure();
+    rl::configure();
     return h;
 }
 
@@ -320,9 +326,12 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
     if (variant == KRATOS_KERNEL_AUTO) variant = auto_variant(h);
     if ((variant == KRATOS_KERNEL_TILED || variant == KRATOS_KERNEL_PAIRED) && !h->tiled_ok)
         return fail(KRATOS_ERR_ARG, "tiled and paired kernels need active x and y axes");
-    if (variant == KRATOS_KERNEL_PAIRED && h->prec != KRATOS_PREC_MIXED)
-        return fail(KRATOS_ERR_ARG, "the paired kernel is the mixed-precision path");
-    if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED && variant != KRATOS_KERNEL_PAIRED)
+    if ((variant == KRATOS_KERNEL_PAIRED || variant == KRATOS_KERNEL_ROLES) && h->prec != KRATOS_PREC_MIXED)
+        return fail(KRATOS_ERR_ARG, "the paired and role-split kernels are the mixed-precision path");
+    if (variant == KRATOS_KERNEL_ROLES && (!h->tiled_ok || !h->g.active[2]))
+        return fail(KRATOS_ERR_ARG, "the role-split kernel needs three active axes");
+    if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED && variant != KRATOS_KERNEL_PAIRED &&
+        variant != KRATOS_KERNEL_ROLES)
         return fail(KRATOS_ERR_ARG, "bad variant");
     h->variant = variant;
     return KRATOS_OK;

@@ -16,8 +16,9 @@ pytestmark = pytest.mark.gpu
 
 P, F, O, R = 0, 1, 2, 3
 MIXED, FP64 = binding.PREC_MIXED, binding.PREC_FP64
-SIMPLE, TILED, PAIRED = binding.KERNEL_SIMPLE, binding.KERNEL_TILED, binding.KERNEL_PAIRED
-KERNELS = [SIMPLE, TILED, PAIRED]
+SIMPLE, TILED, PAIRED, ROLES = (binding.KERNEL_SIMPLE, binding.KERNEL_TILED, binding.KERNEL_PAIRED,
+                                binding.KERNEL_ROLES)
+KERNELS = [SIMPLE, TILED, PAIRED, ROLES]
 TOL = {MIXED: 1e-5, FP64: 1e-12}
 
 
@@ -35,9 +36,11 @@ def rel_l1_fields(got, ref):
 
 
 def make(pr, prec, kernel=binding.KERNEL_AUTO):
-    if kernel == PAIRED and prec != MIXED:
-        pytest.skip("the paired kernel is the mixed-precision path")
+    if kernel in (PAIRED, ROLES) and prec != MIXED:
+        pytest.skip("the paired and role-split kernels are the mixed-precision path")
     nx, ny, nz = pr.shape
+    if kernel == ROLES and min(nx, ny, nz) == 1:
+        pytest.skip("the role-split kernel is the 3D path")
     h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, kernel=kernel)
     h.set_state(pr.U)
     return h
@@ -134,8 +137,8 @@ def test_parity_other_axis_combinations(shape, bc, prec):
     assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
 
 
-@pytest.mark.parametrize("kernel", [TILED, PAIRED])
-@pytest.mark.parametrize("zchunk", [4, 7, 16, 1000])
+@pytest.mark.parametrize("kernel", [TILED, PAIRED, ROLES])
+@pytest.mark.parametrize("zchunk", [1, 2, 4, 7, 16, 1000])
 def test_slab_seams_do_not_change_the_result(zchunk, kernel):
     """Marching slabs of different height must give bit-identical states (one flux per face)."""
     pr = inputs.random_smooth(40, 20, 29, seed=8, gamma=1.4)
@@ -166,7 +169,7 @@ def test_strong_jumps_take_every_hllc_branch():
     dt = 1e-4
     for kernel in KERNELS:
         for prec in (MIXED, FP64):
-            if kernel == PAIRED and prec != MIXED:
+            if kernel in (PAIRED, ROLES) and prec != MIXED:
                 continue
             h = make(pr, prec, kernel)
             h.step(dt)
