@@ -50,11 +50,14 @@ def workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
-def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto") -> str:
+def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto", shape=(0, 0, 0)) -> str:
     """Name of the stage kernel the library launches for this block."""
     if variant == "simple":
         return f"stage_simple<{'float' if prec == 0 else 'double'},{stage}>"
-    if prec == 0 and (variant == "roles" or (variant == "auto" and ndim == 3)):
+    tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0
+    if prec == 0 and (variant == "tma" or (variant == "auto" and tma_ok)):
+        return f"stage_tma<{stage}>"
+    if prec == 0 and variant == "roles":
         return f"stage_roles<{stage}>"
     if prec == 0 and variant in ("auto", "paired"):
         return f"stage_pair<{stage},{ndim}>"
@@ -194,7 +197,7 @@ def run_ours(args):
     ncell = pr.ncell
     stream = torch.cuda.Stream()
     variant = {"auto": binding.KERNEL_AUTO, "simple": binding.KERNEL_SIMPLE, "tiled": binding.KERNEL_TILED,
-               "paired": binding.KERNEL_PAIRED, "roles": binding.KERNEL_ROLES}[args.kernel]
+               "paired": binding.KERNEL_PAIRED, "roles": binding.KERNEL_ROLES, "tma": binding.KERNEL_TMA}[args.kernel]
     h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream, kernel=variant)
     if args.zchunk > 0:
         h.set_zchunk(args.zchunk)
@@ -276,7 +279,7 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
-        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel)
+        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel, (nx, ny, nz))
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                     "unit": "GB/s", "frac": kern[dom]["frac"],
                     "traffic": ncu_traffic(args.workload, args.precision, kname),
@@ -322,7 +325,7 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "roles"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "roles", "tma"],
                     help="stage kernel variant (default: the library's own choice)")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per slab of the marching kernels (0 = auto)")
     args = ap.parse_args()

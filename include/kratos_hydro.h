@@ -65,13 +65,17 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
 #define KRATOS_BC_REFLECT 3  /* q(-i-1/2) = q(i+1/2), normal velocity negated */
 
 /* kernel variants (kratos_hydro_set_kernel) */
-#define KRATOS_KERNEL_AUTO 0   /* x,y active: role-split (mixed, 3D), paired (mixed, 2D) or tiled (all-fp64); else simple */
+#define KRATOS_KERNEL_AUTO 0   /* x,y active: TMA (mixed, 3D, nx % 32 == 0, ny % 16 == 0), else paired (mixed) or tiled
+                                  (all-fp64); otherwise simple */
 #define KRATOS_KERNEL_SIMPLE 1 /* one thread per cell, stencil from global memory (any axes) */
 #define KRATOS_KERNEL_TILED 2  /* shared-memory tile + halo, z marched in registers, each face once */
 #define KRATOS_KERNEL_PAIRED 3 /* mixed precision only: two cells per thread, packed fp32x2 arithmetic,
                                   halo warps, fp64 flux exchange (x,y active) */
 #define KRATOS_KERNEL_ROLES 4  /* mixed precision, three active axes: the paired scheme split over specialised
                                   warps (z march + update | x,y Riemann problems | halo ring) */
+#define KRATOS_KERNEL_TMA 5    /* the paired scheme with all global traffic moved by TMA boxes (a producer warp loads
+                                  tile, halo and U0 planes onto mbarriers and stores each updated plane): mixed
+                                  precision, three active axes, nx % 32 == 0, ny % 16 == 0 */
 
 /* Create a solver for an nx*ny*nz block.  gamma > 1.  bc (host, 6 ints) =
  * {x-lo, x-hi, y-lo, y-hi, z-lo, z-hi}; periodic must be set on both sides of an axis or

@@ -18,7 +18,7 @@ from . import build as _build
 
 PREC_MIXED, PREC_FP64 = 0, 1
 BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
-KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_ROLES = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_ROLES, KERNEL_TMA = 0, 1, 2, 3, 4, 5
 OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
 
 # every symbol include/kratos_hydro.h declares

@@ -15,6 +15,7 @@
 #include "kh_tiled.cuh"
 #include "kh_pair.cuh"
 #include "kh_role.cuh"
+#include "kh_tma.cuh"
 
 using namespace kh;
 
@@ -46,6 +47,7 @@ struct kratos_hydro {
     int variant;     // resolved KRATOS_KERNEL_SIMPLE / _TILED
     bool tiled_ok;   // tiled kernel supports this block
     int zchunk;      // 0 = auto
+    tma::StageMaps* maps;  // tensor maps of the TMA kernel (host; NULL when the block is not supported)
     double* U0;      // current state (device)
     double* U1;      // predictor (device)
     Ctrl* ctrl;      // device
@@ -117,13 +119,15 @@ int auto_variant(const kratos_hydro* h)
 {
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
-    return h->g.active[2] ? KRATOS_KERNEL_ROLES : KRATOS_KERNEL_PAIRED;
+    if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
+    return KRATOS_KERNEL_PAIRED;  // fastest measured on B200
 }
 
 int pick_zchunk(const kratos_hydro* h)
 {
     if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
-    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES) ? pr::auto_zchunk(h->g)
+    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES || h->variant == KRATOS_KERNEL_TMA)
+               ? pr::auto_zchunk(h->g)
                                                                                       : tiled_auto_zchunk(h->g);
 }
 
@@ -134,7 +138,9 @@ int launch_stage(kratos_hydro* h, int stage)
     const double* Uin = (stage == 1) ? h->U0 : h->U1;
     double* Uout = (stage == 1) ? h->U1 : h->U0;
     LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
-    if (h->variant == KRATOS_KERNEL_ROLES) {
+    if (h->variant == KRATOS_KERNEL_TMA) {
+        tma::launch_stage(stage, *h->maps, g, h->ctrl, pick_zchunk(h), h->stream);
+    } else if (h->variant == KRATOS_KERNEL_ROLES) {
         rl::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_PAIRED) {
         pr::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
@@ -256,6 +262,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     g.gamma = gamma;
     h->prec = prec;
     h->tiled_ok = g.active[0] && g.active[1];
+    h->maps = nullptr;
     h->variant = auto_variant(h);
     h->zchunk = 0;
     h->stream = 0;
@@ -285,6 +292,12 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     tiled_configure();
     pr::configure();
     rl::configure();
+    tma::configure();
+    if (prec == KRATOS_PREC_MIXED && tma::supported(g)) {
+        h->maps = new (std::nothrow) tma::StageMaps;
+        if (h->maps) tma::build_maps(h->maps, h->U0, h->U1, g);
+    }
+    h->variant = auto_variant(h);
     return h;
 }
 
@@ -298,6 +311,7 @@ void kratos_hydro_destroy(kratos_hydro_t* h)
     cudaFree(h->d_tot);
     cudaFree(h->p_partial);
     if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
+    delete h->maps;
     for (auto e : h->ev_pool) cudaEventDestroy(e);
     delete h;
 }
@@ -330,8 +344,10 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
         return fail(KRATOS_ERR_ARG, "the paired and role-split kernels are the mixed-precision path");
     if (variant == KRATOS_KERNEL_ROLES && (!h->tiled_ok || !h->g.active[2]))
         return fail(KRATOS_ERR_ARG, "the role-split kernel needs three active axes");
+    if (variant == KRATOS_KERNEL_TMA && !(h->maps && h->maps->ok))
+        return fail(KRATOS_ERR_ARG, "the TMA kernel needs mixed precision, three active axes, nx %% 32 == 0 and ny %% 16 == 0");
     if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED && variant != KRATOS_KERNEL_PAIRED &&
-        variant != KRATOS_KERNEL_ROLES)
+        variant != KRATOS_KERNEL_ROLES && variant != KRATOS_KERNEL_TMA)
         return fail(KRATOS_ERR_ARG, "bad variant");
     h->variant = variant;
     return KRATOS_OK;

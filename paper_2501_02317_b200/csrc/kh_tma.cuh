@@ -1,0 +1,643 @@
+// kh_tma.cuh -- KRATOS_KERNEL_TMA: the paired Heun-stage kernel (kh_pair.cuh) with every byte of global
+// traffic moved by the Tensor Memory Accelerator (3D blocks, mixed precision, nx % 32 == 0, ny % 16 == 0).
+//
+// The arithmetic is that of kh_pair.cuh, function for function (recover, plm, hllc2: PAPER.md:163-173,
+// Eq. 3, Eq. 4-5; fp64 update and Heun average: PAPER.md:232-238, 264).  What changes is how the conserved
+// state gets on and off the chip.  In the paired kernel one third of the issue slots of a main warp went
+// into 8-byte cp.async copies, 64-bit address arithmetic, boundary-rule branches and predicated stores.
+// Here a producer warp issues, per plane of the z march,
+//     one 4-D TMA box (32 x 16 x 1 x 5 doubles) for the tile,          -> raw[slot]
+//     four boxes for the 2-cell halo (two row pairs, two column pairs)   -> hrow / hcol[slot]
+//     one box for U0 of the plane being averaged (stage 2)               -> u0[slot]
+// each completing on an mbarrier, and one TMA store per plane: the main warps write the new state over the
+// raw state they just consumed (in place, same addresses, no extra buffer) and the producer ships the box.
+// The main warps contain no global-memory instruction at all, the halo warps read their cells from shared
+// memory, and the boundary rules of Sec. 3.1.1 become a choice of box coordinates
+// (periodic wrap, clamp, mirror) made once per block plus the normal-velocity rule applied at conversion.
+//
+// Phases per plane k (as in kh_pair.cuh):
+//   A) x/y slopes from the primitive tile, left states published            | barrier 1
+//      [producer: store plane k-1, then refill its slot with plane k-1+NSLOT; halo plane k+3; U0(k+1)]
+//   B) z/x/y fluxes of plane k, conversion of plane k+2, tile of plane k+1   | barrier 2
+//   C) fp64 update of plane k, written in place; Heun average and CFL rate (stage 2)
+#pragma once
+#include <cuda.h>
+
+#include "kh_pair.cuh"
+
+namespace kh {
+namespace tma {
+
+using pr::f2;
+using pr::mk;
+using pr::plm;
+using pr::face_flux2;
+using pr::recover;
+using pr::Gas;
+
+constexpr int PTX = pr::PTX;       // 32
+constexpr int PTY = pr::PTY;       // 16
+constexpr int PRP = pr::PRP;       // 8 row pairs = main warps
+constexpr int WARP_HALO_Y = PRP;
+constexpr int WARP_HALO_X = PRP + 1;
+constexpr int WARP_PRODUCER = PRP + 2;
+constexpr int NWARPS = PRP + 4;        // two main warpgroups + one auxiliary warpgroup (halo y, halo x, producer, idle):
+                                       // setmaxnreg acts on whole warpgroups
+constexpr int NTHREADS = NWARPS * 32;
+constexpr int NHALO = 3;           // halo ring depth
+#define KH_TMA_MAIN_REGS "184"
+#define KH_TMA_HALO_REGS "136"
+
+template <int STAGE>
+struct Cfg {
+    static constexpr int NSLOT = (STAGE == 1) ? 5 : 4;   // raw ring depth (stage 2 shares the space with U0)
+    static constexpr int NU0 = (STAGE == 2) ? 2 : 0;
+};
+
+constexpr int OWN_BYTES = 5 * PTY * PTX * 8;    // one tile box
+constexpr int ROW_BYTES = 5 * 2 * PTX * 8;      // one halo row pair
+constexpr int COL_BYTES = 5 * PTY * 2 * 8;      // one halo column pair
+
+template <int STAGE>
+struct Smem {
+    static constexpr int NSLOT = Cfg<STAGE>::NSLOT;
+    alignas(128) double raw[NSLOT][5][PTY][PTX];              // fp64 state of the tile, planes in flight
+    alignas(128) double u0[(STAGE == 2) ? 2 : 1][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
+    alignas(128) double hrow[NHALO][2][5][2][PTX];            // halo rows: [lo/hi][field][box row][column]
+    alignas(128) double hcol[NHALO][2][5][PTY][2];            // halo columns: [lo/hi][field][row][box column]
+    f2 Wt[5][PRP + 2][PTX + 4];                               // primitives of one plane, row pairs -1..PRP, columns -2..PTX+1
+    f2 QLx[5][PRP][PTX + 1];                                  // left states at x faces c = 0..PTX (from column c-1)
+    f2 QRxR[5][PRP];                                          // right state at x face PTX (from halo column PTX)
+    float QLy[5][PRP + 1][PTX];                               // left states at y faces r = 0..PRP (from row 2r-1)
+    float QRyT[5][PTX];                                       // right state at y face PRP (from halo row PTY)
+    double2 Fx[5][PRP][PTX + 1];                              // fp64 fluxes through x faces
+    double Fy[5][PRP + 1][PTX];                               // fp64 fluxes through the y faces between row pairs
+    double red[32];
+    unsigned long long full_raw[NSLOT];
+    unsigned long long full_halo[NHALO];
+    unsigned long long full_u0[2];
+};
+
+// tensor maps of one stage launch (64-byte aligned kernel parameters)
+struct Maps {
+    CUtensorMap in_own, in_rows, in_cols;   // stage input: tile box, halo row pair, halo column pair
+    CUtensorMap u0_own;                     // U0 (stage 2)
+    CUtensorMap out_own;                    // stage output
+};
+
+// ---- PTX wrappers -------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_parity(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra D_%=;\n\t"
+        "bra W_%=;\n\t"
+        "D_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load4(void* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                          unsigned long long* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::
+            "r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void tma_store4(const CUtensorMap* map, int c0, int c1, int c2, int c3, const void* src)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(map),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src))
+                 : "memory");
+}
+__device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "memory"); }
+
+// Where the two halo cells beyond one side of the tile come from (Sec. 3.1.1): first source coordinate of the
+// 2-wide box, the position inside the box of each of the two cells, and the normal-velocity rule.
+// (Tiles start at multiples of 16 and extents are even, so the smaller source coordinate is even except for
+// the clamp onto cell n-1 of the Free / Outflow rules, where both cells sit at position 1 of the box.)
+struct HaloSide {
+    int start, idx0, idx1, rule;
+};
+__device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_hi)
+{
+    int r0, r1;
+    const int s0 = bc_source(c0, n, bc_lo, bc_hi, r0);
+    const int s1 = bc_source(c0 + 1, n, bc_lo, bc_hi, r1);
+    HaloSide h;
+    h.start = min(s0, s1) & ~1;  // even: the box stays inside the block and its first byte 16-byte aligned
+    h.idx0 = s0 - h.start;
+    h.idx1 = s1 - h.start;
+    h.rule = r0;  // both cells lie beyond the same face
+    return h;
+}
+
+// One Heun stage.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin + dt L(Uin))
+// (Uout aliases U0) and the CFL rate maximum of Uout.  3D only.
+template <int STAGE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
+{
+    using S = Smem<STAGE>;
+    constexpr int NSLOT = S::NSLOT;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    S& sm = *reinterpret_cast<S*>(smem_raw);
+
+    const double dt = ctrl->dt;
+    if (!(dt > 0.0)) return;  // a step clipped to zero length (run_until past t_end) does nothing
+    const double pref_d = ctrl->p_ref;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int i0 = blockIdx.x * PTX, j0 = blockIdx.y * PTY;
+    const int kbeg = blockIdx.z * zchunk;
+    const int kend = min(kbeg + zchunk, nz);
+    const int kfirst = kbeg - 1;  // priming iteration: builds the tile of plane kbeg
+    const int pbase = kbeg - 2;   // first plane of the raw ring: plane p sits in slot (p - pbase) % NSLOT
+    const double gm1 = g.gamma - 1.0;
+    Gas gas;
+    gas.gamma = (float)g.gamma;
+    gas.g1 = (float)((g.gamma + 1.0) / (2.0 * g.gamma));
+    gas.igm1 = (float)(1.0 / (g.gamma - 1.0));
+    gas.pref = (float)pref_d;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSLOT; s++) mbar_init(&sm.full_raw[s], 1);
+        for (int s = 0; s < NHALO; s++) mbar_init(&sm.full_halo[s], 1);
+        mbar_init(&sm.full_u0[0], 1);
+        mbar_init(&sm.full_u0[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    int hits = 0;
+    f2 rate = mk(0.0f, 0.0f);
+
+    if (warp < PRP) {
+        // ================================ main warps: cells (i, ja), (i, ja+1) ========================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 " KH_TMA_MAIN_REGS ";");
+        const int w = warp;
+        constexpr int RAWF = PTY * PTX, RAWS = 5 * RAWF;              // double strides of raw / u0: field, slot
+        constexpr int WTF = (PRP + 2) * (PTX + 4);                    // f2 field stride of Wt
+        constexpr int QXF = PRP * (PTX + 1);                          // f2 field stride of QLx, double2 of Fx
+        constexpr int QYF = (PRP + 1) * PTX;                          // field stride of QLy (float) and Fy (double)
+        double* const raw0 = &sm.raw[0][0][2 * w][lane];              // row 2w; row 2w+1 is + PTX
+        const double* const u00 = &sm.u0[0][0][(STAGE == 2) ? 2 * w : 0][lane];
+        f2* const wt = &sm.Wt[0][w + 1][lane + 2];
+        f2* const qlx = &sm.QLx[0][w][lane];      // left state of the own low x face; own high face is + 1
+        float* const qly = &sm.QLy[0][w][lane];   // left state of the pair's low y face; the pair's high face is + PTX
+        double2* const fxs = &sm.Fx[0][w][lane];
+        double* const fys = &sm.Fy[0][w][lane];
+
+        const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1], dtdz = dt * g.inv_dx[2];
+        const CflConst<float> cc(g);
+
+        // conversion of plane kk (ring index q = kk - pbase): wait for its box, recover the pair's primitives
+        auto convert = [&](int kk, int slot, unsigned parity, f2 W[5], bool count) {
+            int rz = VN_KEEP;
+            if (kk < 0 || kk >= nz) (void)bc_source(kk, nz, g.bc[4], g.bc[5], rz);
+            mbar_wait_parity(&sm.full_raw[slot], parity);
+            const double* s = raw0 + slot * RAWS;
+            double ua[5], ub[5];
+#pragma unroll
+            for (int f = 0; f < 5; f++) { ua[f] = s[f * RAWF]; ub[f] = s[f * RAWF + PTX]; }
+            float Wa[5], Wb[5];
+            const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, VN_KEEP, VN_KEEP, rz, Wa);
+            const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, VN_KEEP, VN_KEEP, rz, Wb);
+            if (count) hits += ha + hb;
+#pragma unroll
+            for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
+        };
+
+        // ---- prologue: planes kbeg-2, kbeg-1, kbeg (ring slots 0, 1, 2, first fill: parity 0) ----
+        f2 Wa[5], Wb[5], QLz[5];   // W(k), W(k+1), left state of z face k+1/2
+        double2 Fzlo[5];           // dt/dz * flux through z face k-1/2
+        {
+            f2 Wm[5];
+            convert(kbeg - 2, 0, 0u, Wm, false);
+            convert(kbeg - 1, 1, 0u, Wa, false);
+            convert(kbeg, 2, 0u, Wb, true);
+#pragma unroll
+            for (int f = 0; f < 5; f++) {
+                f2 qR;
+                plm(Wm[f], Wa[f], Wb[f], QLz[f], qR);
+                Fzlo[f] = make_double2(0.0, 0.0);
+            }
+        }
+        // ring positions of the planes k+2 (converted) and k (updated) at the first iteration k = kfirst
+        int s_conv = 3 % NSLOT, s_upd = 1;
+        unsigned par_conv = (3 >= NSLOT) ? 1u : 0u;
+
+        f2 QRx[5], QRy[5];
+        float QLyo[5];  // left state of the face between the pair's two cells
+        double2 dU[5];
+#pragma unroll
+        for (int f = 0; f < 5; f++) { QRx[f] = QRy[f] = mk(0.f, 0.f); QLyo[f] = 0.f; dU[f] = make_double2(0.0, 0.0); }
+
+#pragma unroll 1
+        for (int k = kfirst; k < kend; k++) {
+            const bool live = k >= kbeg;
+            // ---------------- phase A: x / y slopes of plane k from the tile ----------------
+            if (live) {
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const f2 q = Wa[f];
+                    f2 qL;
+                    plm(wt[f * WTF - 1], q, wt[f * WTF + 1], qL, QRx[f]);
+                    qlx[f * QXF + 1] = qL;
+                    const f2 below = wt[f * WTF - (PTX + 4)], above = wt[f * WTF + (PTX + 4)];
+                    f2 qLy;
+                    plm(mk(below.y, q.x), q, mk(q.y, above.x), qLy, QRy[f]);
+                    QLyo[f] = qLy.x;
+                    qly[f * QYF + PTX] = qLy.y;
+                }
+            }
+            block_bar();
+            // ---------------- phase B: fluxes of plane k, tile of plane k+1 ----------------
+            f2 Wn[5];
+            double2 Fzhi[5];
+            {
+                convert(k + 2, s_conv, par_conv, Wn, k + 2 < kend);
+                f2 qL[5], qR[5], F[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    qL[f] = QLz[f];
+                    plm(Wa[f], Wb[f], Wn[f], QLz[f], qR[f]);
+                }
+                face_flux2<2>(qL, qR, gas, F);
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    Fzhi[f] = make_double2(dtdz * (double)F[f].x, dtdz * (double)F[f].y);
+                    dU[f] = make_double2(Fzlo[f].x - Fzhi[f].x, Fzlo[f].y - Fzhi[f].y);
+                }
+            }
+            if (live) {
+                {
+                    f2 qL[5], F[5];
+#pragma unroll
+                    for (int f = 0; f < 5; f++) qL[f] = qlx[f * QXF];
+                    face_flux2<0>(qL, QRx, gas, F);
+#pragma unroll
+                    for (int f = 0; f < 5; f++) {
+                        const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
+                        fxs[f * QXF] = fd;
+                        dU[f].x = fma(dtdx, fd.x, dU[f].x);
+                        dU[f].y = fma(dtdx, fd.y, dU[f].y);
+                    }
+                }
+                {
+                    f2 qL[5], F[5];
+#pragma unroll
+                    for (int f = 0; f < 5; f++) qL[f] = mk(qly[f * QYF], QLyo[f]);
+                    face_flux2<1>(qL, QRy, gas, F);
+#pragma unroll
+                    for (int f = 0; f < 5; f++) {
+                        const double flo = (double)F[f].x, fin = (double)F[f].y;
+                        fys[f * QYF] = flo;
+                        dU[f].x = fma(dtdy, flo - fin, dU[f].x);
+                        dU[f].y = fma(dtdy, fin, dU[f].y);
+                    }
+                }
+            }
+            if (k + 1 < kend) {
+#pragma unroll
+                for (int f = 0; f < 5; f++) wt[f * WTF] = Wb[f];
+            }
+            block_bar();
+            // ---------------- phase C: fp64 update of plane k, in place ----------------
+            if (live) {
+                double* su = raw0 + s_upd * RAWS;
+                const double* s0 = u00 + ((k - kbeg) & 1) * RAWS;
+                if (STAGE == 2) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
+                double ua[5], ub[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const double2 fxh = fxs[f * QXF + 1];
+                    const double fyh = fys[f * QYF + PTX];
+                    double xa = su[f * RAWF] + fma(-dtdx, fxh.x, dU[f].x);
+                    double xb = su[f * RAWF + PTX] + fma(-dtdy, fyh, fma(-dtdx, fxh.y, dU[f].y));
+                    if (STAGE == 2) {
+                        xa = 0.5 * s0[f * RAWF] + 0.5 * xa;
+                        xb = 0.5 * s0[f * RAWF + PTX] + 0.5 * xb;
+                    }
+                    ua[f] = xa;
+                    ub[f] = xb;
+                    su[f * RAWF] = xa;
+                    su[f * RAWF + PTX] = xb;
+                }
+                fence_async_smem();  // the producer ships this box after the next barrier
+                if (STAGE == 2) {
+                    float ra = cfl_rate_from_cons<float>(ua, cc);
+                    float rb = cfl_rate_from_cons<float>(ub, cc);
+                    if (!(ra == ra)) ra = __int_as_float(0x7f800000);
+                    if (!(rb == rb)) rb = __int_as_float(0x7f800000);
+                    rate = mk(fmaxf(rate.x, ra), fmaxf(rate.y, rb));
+                }
+            }
+            // rotate the z march and the ring
+#pragma unroll
+            for (int f = 0; f < 5; f++) { Wa[f] = Wb[f]; Wb[f] = Wn[f]; Fzlo[f] = Fzhi[f]; }
+            if (++s_conv == NSLOT) { s_conv = 0; par_conv ^= 1u; }
+            if (++s_upd == NSLOT) s_upd = 0;
+        }
+        block_bar();  // the producer ships the last plane after this barrier
+    } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 " KH_TMA_HALO_REGS ";");
+    if (warp == WARP_HALO_Y) {
+        // ================================ halo rows -2, -1, PTY, PTY+1 (lane = column) ==================
+        const HaloSide lo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
+        const HaloSide hi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
+        constexpr int HF = 2 * PTX, HSIDE = 5 * HF, HSLOT = 2 * HSIDE;   // double strides of hrow: field, side, slot
+        const int off[4] = {lo.idx0 * PTX + lane, lo.idx1 * PTX + lane, HSIDE + hi.idx0 * PTX + lane,
+                            HSIDE + hi.idx1 * PTX + lane};
+        const int ry[4] = {lo.rule, lo.rule, hi.rule, hi.rule};
+        const double* const h0 = &sm.hrow[0][0][0][0][0];
+        constexpr int WTF = (PRP + 2) * (PTX + 4);
+        constexpr int QYF = (PRP + 1) * PTX;
+        f2* const wlo = &sm.Wt[0][0][lane + 2];          // rows -2, -1
+        f2* const whi = &sm.Wt[0][PRP + 1][lane + 2];    // rows PTY, PTY+1
+        float W[4][5];
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+#pragma unroll
+            for (int f = 0; f < 5; f++) W[r][f] = 0.0f;
+        int hs = 0;
+        unsigned hpar = 0u;
+#pragma unroll 1
+        for (int k = kfirst; k < kend; k++) {
+            const bool live = k >= kbeg;
+            // phase A: limited y states of rows -1 and PTY of plane k
+            if (live) {
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const f2 r01 = wlo[f * WTF + (PTX + 4)];        // rows 0, 1
+                    const f2 rtop = whi[f * WTF - (PTX + 4)];       // rows PTY-2, PTY-1
+                    f2 qL, qR;
+                    plm(mk(W[0][f], rtop.y), mk(W[1][f], W[2][f]), mk(r01.x, W[3][f]), qL, qR);
+                    sm.QLy[f][0][lane] = qL.x;    // row -1: left state of the tile's low y face
+                    sm.QRyT[f][lane] = qR.y;      // row PTY: right state of the tile's high y face
+                }
+            }
+            block_bar();
+            // phase B: flux through the tile's high y face of plane k; halo rows of plane k+1
+            if (live) {
+                f2 qL[5], qR[5], F[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const float l = sm.QLy[f][PRP][lane], r = sm.QRyT[f][lane];
+                    qL[f] = mk(l, l);
+                    qR[f] = mk(r, r);
+                }
+                face_flux2<1>(qL, qR, gas, F);
+#pragma unroll
+                for (int f = 0; f < 5; f++) sm.Fy[f][PRP][lane] = (double)F[f].x;
+            }
+            if (k + 1 < kend) {
+                mbar_wait_parity(&sm.full_halo[hs], hpar);
+                const double* s = h0 + hs * HSLOT;
+#pragma unroll
+                for (int r = 0; r < 4; r++) {
+                    double u[5];
+#pragma unroll
+                    for (int f = 0; f < 5; f++) u[f] = s[off[r] + f * HF];
+                    (void)recover(u[0], u[1], u[2], u[3], u[4], gm1, pref_d, VN_KEEP, ry[r], VN_KEEP, W[r]);
+                }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    wlo[f * WTF] = mk(W[0][f], W[1][f]);
+                    whi[f * WTF] = mk(W[2][f], W[3][f]);
+                }
+                if (++hs == NHALO) { hs = 0; hpar ^= 1u; }
+            }
+            block_bar();
+        }
+        block_bar();
+    } else if (warp == WARP_HALO_X) {
+        // ================================ halo columns -2, -1, PTX, PTX+1 =============================
+        const int cid = lane & 3, rp = lane >> 2;                   // column id, row pair
+        const int col = (cid < 2) ? cid - 2 : PTX + cid - 2;
+        const HaloSide side = (cid < 2) ? halo_side(i0 - 2, nx, g.bc[0], g.bc[1]) : halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
+        const int bidx = (cid & 1) ? side.idx1 : side.idx0;
+        const int rx = side.rule;
+        constexpr int CF = PTY * 2, CSIDE = 5 * CF, CSLOT = 2 * CSIDE;   // double strides of hcol: field, side, slot
+        const double* const c0 = &sm.hcol[0][0][0][0][0] + (cid >> 1) * CSIDE + (2 * rp) * 2 + bidx;
+        constexpr int WTF = (PRP + 2) * (PTX + 4);
+        f2* const wt = &sm.Wt[0][rp + 1][col + 2];
+        const int dl = (cid == 0) ? 0 : -1, dr = (cid == 3) ? 0 : 1;   // neighbours inside the tile array
+        f2 W[5];
+#pragma unroll
+        for (int f = 0; f < 5; f++) W[f] = mk(0.f, 0.f);
+        int hs = 0;
+        unsigned hpar = 0u;
+#pragma unroll 1
+        for (int k = kfirst; k < kend; k++) {
+            const bool live = k >= kbeg;
+            // phase A: limited x states of columns -1 and PTX of plane k
+            if (live) {
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    f2 qL, qR;
+                    plm(wt[f * WTF + dl], W[f], wt[f * WTF + dr], qL, qR);
+                    if (cid == 1) sm.QLx[f][rp][0] = qL;   // column -1: left state of the tile's low x face
+                    if (cid == 2) sm.QRxR[f][rp] = qR;     // column PTX: right state of the tile's high x face
+                }
+            }
+            block_bar();
+            // phase B: flux through the tile's high x face of plane k; halo columns of plane k+1
+            if (live && cid == 2) {
+                f2 qL[5], qR[5], F[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) { qL[f] = sm.QLx[f][rp][PTX]; qR[f] = sm.QRxR[f][rp]; }
+                face_flux2<0>(qL, qR, gas, F);
+#pragma unroll
+                for (int f = 0; f < 5; f++) sm.Fx[f][rp][PTX] = make_double2((double)F[f].x, (double)F[f].y);
+            }
+            if (k + 1 < kend) {
+                mbar_wait_parity(&sm.full_halo[hs], hpar);
+                const double* s = c0 + hs * CSLOT;
+                double ua[5], ub[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) { ua[f] = s[f * CF]; ub[f] = s[f * CF + 2]; }
+                float Wa[5], Wb[5];
+                (void)recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wa);
+                (void)recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wb);
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    W[f] = mk(Wa[f], Wb[f]);
+                    wt[f * WTF] = W[f];
+                }
+                if (++hs == NHALO) { hs = 0; hpar ^= 1u; }
+            }
+            block_bar();
+        }
+        block_bar();
+    } else if (warp == WARP_PRODUCER) {
+        // ================================ producer warp: all global traffic, by TMA =====================
+        const HaloSide ylo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
+        const HaloSide yhi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
+        const HaloSide xlo = halo_side(i0 - 2, nx, g.bc[0], g.bc[1]);
+        const HaloSide xhi = halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
+        const int plast = kend + 1;  // last plane the z stencil of this slab needs
+        auto load_raw = [&](int p, int slot) {
+            int rz;
+            const int sk = bc_source(p, nz, g.bc[4], g.bc[5], rz);
+            mbar_expect_tx(&sm.full_raw[slot], OWN_BYTES);
+            tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);
+        };
+        auto load_halo = [&](int p, int slot) {  // p in [kbeg, kend): an interior plane
+            unsigned long long* bar = &sm.full_halo[slot];
+            mbar_expect_tx(bar, 2 * ROW_BYTES + 2 * COL_BYTES);
+            tma_load4(&sm.hrow[slot][0][0][0][0], &maps.in_rows, i0, ylo.start, p, 0, bar);
+            tma_load4(&sm.hrow[slot][1][0][0][0], &maps.in_rows, i0, yhi.start, p, 0, bar);
+            tma_load4(&sm.hcol[slot][0][0][0][0], &maps.in_cols, xlo.start, j0, p, 0, bar);
+            tma_load4(&sm.hcol[slot][1][0][0][0], &maps.in_cols, xhi.start, j0, p, 0, bar);
+        };
+        if (lane == 0) {
+            for (int q = 0; q < NSLOT; q++)
+                if (pbase + q <= plast) load_raw(pbase + q, q);
+            for (int m = 0; m < NHALO; m++)
+                if (kbeg + m < kend) load_halo(kbeg + m, m);
+        }
+        int s_prev = 0;   // ring slot of plane k-1 (plane kbeg-2 at the first iteration)
+        int hs = 0;       // halo slot of plane k (for k >= kbeg)
+#pragma unroll 1
+        for (int k = kfirst; k < kend; k++) {
+            __syncwarp();
+            block_bar();
+            if (lane == 0) {
+                const bool stored = k - 1 >= kbeg;
+                if (stored) {  // plane k-1 was updated in place in phase C of the previous iteration
+                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.raw[s_prev][0][0][0]);
+                    tma_commit();
+                }
+                if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
+                if (STAGE == 2 && k + 1 < kend) {
+                    const int m = (k + 1 - kbeg) & 1;
+                    mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
+                    tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
+                }
+                const int p = k - 1 + NSLOT;
+                if (p <= plast) {
+                    if (stored) tma_wait_read0();  // the store has read the box: the slot may be refilled
+                    load_raw(p, s_prev);
+                }
+            }
+            if (++s_prev == NSLOT) s_prev = 0;
+            if (k >= kbeg && ++hs == NHALO) hs = 0;
+            __syncwarp();
+            block_bar();
+        }
+        __syncwarp();
+        block_bar();
+        if (lane == 0) {  // the last plane of the slab
+            tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.raw[s_prev][0][0][0]);
+            tma_commit();
+            tma_wait_all0();
+        }
+        __syncwarp();
+    } else {
+        // the fourth warp of the auxiliary warpgroup only keeps the barriers
+#pragma unroll 1
+        for (int k = kfirst; k < kend; k++) { block_bar(); block_bar(); }
+        block_bar();
+    }
+    }
+
+    if (hits) atomicAdd(&ctrl->floor_hits, (unsigned long long)hits);
+    if (STAGE == 2) {
+        __syncthreads();
+        block_atomic_max_nonneg((double)fmaxf(rate.x, rate.y), &ctrl->rate_bits, sm.red);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link against libcuda)
+inline EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// Tensor map over one conserved state U[5][nz][ny][nx] (fp64, x fastest) with a box of bx x by x 1 x 5.
+inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx, int by)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2], 5};
+    const cuuint64_t strides[3] = {(cuuint64_t)g.n[0] * 8, (cuuint64_t)g.n[0] * g.n[1] * 8, (cuuint64_t)g.N * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 5};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// maps of both stages for the two state buffers of a handle: stage 1 reads A writes B, stage 2 reads B, averages with
+// and writes A.
+struct StageMaps {
+    Maps s1, s2;
+    bool ok;
+};
+
+inline bool supported(const Grid& g)
+{
+    return g.active[0] && g.active[1] && g.active[2] && g.n[0] % PTX == 0 && g.n[1] % PTY == 0 && g.n[2] >= 2 &&
+           (g.N * 8) % 16 == 0 && (unsigned long long)g.N * 8 < (1ull << 40);
+}
+
+inline void build_maps(StageMaps* sm, const double* A, const double* B, const Grid& g)
+{
+    sm->ok = false;
+    if (!supported(g)) return;
+    CUtensorMap a_own, a_rows, a_cols, b_own, b_rows, b_cols;
+    if (!make_map(&a_own, A, g, PTX, PTY) || !make_map(&a_rows, A, g, PTX, 2) || !make_map(&a_cols, A, g, 2, PTY) ||
+        !make_map(&b_own, B, g, PTX, PTY) || !make_map(&b_rows, B, g, PTX, 2) || !make_map(&b_cols, B, g, 2, PTY))
+        return;
+    sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = b_own;
+    sm->s2.in_own = b_own; sm->s2.in_rows = b_rows; sm->s2.in_cols = b_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
+    sm->ok = true;
+}
+
+inline int auto_zchunk(const Grid& g) { return pr::auto_zchunk(g); }
+
+inline void configure()
+{
+    static_assert(sizeof(Smem<1>) + 128 <= 227 * 1024 && sizeof(Smem<2>) + 128 <= 227 * 1024,
+                  "tile does not fit the shared memory of one SM");
+    cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
+    cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
+inline void launch_stage(int stage, const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
+{
+    dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
+    if (stage == 1) stage_tma<1><<<grid, NTHREADS, sizeof(Smem<1>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
+    else            stage_tma<2><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
+}
+
+}  // namespace tma
+}  // namespace kh
