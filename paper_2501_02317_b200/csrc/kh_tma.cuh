@@ -35,6 +35,9 @@ using pr::face_flux2;
 using pr::recover;
 using pr::Gas;
 
+#ifndef KH_TMA_UNROLL
+#define KH_TMA_UNROLL 2
+#endif
 constexpr int PTX = pr::PTX;       // 32
 constexpr int PTY = pr::PTY;       // 16
 constexpr int PRP = pr::PRP;       // 8 row pairs = main warps
@@ -45,8 +48,16 @@ constexpr int NWARPS = PRP + 4;        // two main warpgroups + one auxiliary wa
                                        // setmaxnreg acts on whole warpgroups
 constexpr int NTHREADS = NWARPS * 32;
 constexpr int NHALO = 3;           // halo ring depth
-#define KH_TMA_MAIN_REGS "184"
-#define KH_TMA_HALO_REGS "136"
+constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (register rotation becomes renaming)
+// register split of the three warpgroups (setmaxnreg): per scheduler 2 main warps + 1 auxiliary warp <= 16384
+#ifndef KH_TMA_MAIN_REGS
+#define KH_TMA_MAIN_REGS 184
+#endif
+#ifndef KH_TMA_HALO_REGS
+#define KH_TMA_HALO_REGS 136
+#endif
+#define KH_TMA_STR2(x) #x
+#define KH_TMA_STR(x) KH_TMA_STR2(x)
 
 template <int STAGE>
 struct Cfg {
@@ -143,6 +154,114 @@ __device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_h
     return h;
 }
 
+// pr::hllc2 (Sec. 3.2.2; formulas documented at kh::hllc) for N independent face pairs in
+// lock step: every statement is issued for all N before the next one, so that the N dependency chains are
+// interleaved in program order and the fixed latencies of one hide behind the others.  Operation for operation
+// the same arithmetic as pr::hllc2, hence the same bits.
+template <int N>
+__device__ __forceinline__ void hllc2n(const f2 (&L)[N][5], const f2 (&R)[N][5], const Gas& g, f2 (&F)[N][5])
+{
+    using namespace pr;
+    const f2 pref = bc(g.pref), one = bc(1.0f);
+#define KH_EACH for (int n = 0; n < N; n++)
+    f2 pL[N], pR[N], gpL[N], gpR[N], cL[N], cR[N], w[N], pst[N], qL[N], qR[N], dsL[N], dsR[N], mL[N], mR[N];
+    f2 num[N], den[N], sL[N], rK[N], pKd[N], uK[N], vK[N], wK[N], dsK[N], mK[N], pK[N], sK[N], D[N], r[N];
+    f2 sst[N], inv[N], ke[N], EK[N], phi[N], pstKd[N], F0[N], F1[N], A4[N], F4[N], G0[N], G1[N], G4[N];
+    bool lx[N], ly[N], ox[N], oy[N];
+#pragma unroll
+    KH_EACH { pL[n] = add2(L[n][1], pref); pR[n] = add2(R[n][1], pref); }
+#pragma unroll
+    KH_EACH { gpL[n] = mul2(bc(g.gamma), pL[n]); gpR[n] = mul2(bc(g.gamma), pR[n]); }
+#pragma unroll
+    KH_EACH { cL[n] = mul2(gpL[n], rsqrt2(mul2(gpL[n], L[n][0]))); cR[n] = mul2(gpR[n], rsqrt2(mul2(gpR[n], R[n][0]))); }
+#pragma unroll
+    KH_EACH w[n] = mul2(mul2(sub2(R[n][2], L[n][2]), add2(L[n][0], R[n][0])), add2(cL[n], cR[n]));
+#pragma unroll
+    KH_EACH pst[n] = maxs(fma2(bc(-0.125f), w[n], mul2(bc(0.5f), add2(L[n][1], R[n][1]))), -g.pref);
+#pragma unroll
+    KH_EACH {
+        qL[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], L[n][1]), rcp2(pL[n]))), one));
+        qR[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], R[n][1]), rcp2(pR[n]))), one));
+    }
+#pragma unroll
+    KH_EACH { dsL[n] = neg2(mul2(cL[n], qL[n])); dsR[n] = mul2(cR[n], qR[n]); }
+#pragma unroll
+    KH_EACH { mL[n] = mul2(L[n][0], dsL[n]); mR[n] = mul2(R[n][0], dsR[n]); }
+#pragma unroll
+    KH_EACH {
+        num[n] = sub2(fma2(neg2(mR[n]), R[n][2], R[n][1]), fma2(neg2(mL[n]), L[n][2], L[n][1]));
+        den[n] = sub2(mL[n], mR[n]);
+        sL[n] = add2(L[n][2], dsL[n]);
+    }
+#pragma unroll
+    KH_EACH {
+        lx[n] = (sL[n].x >= 0.0f) || (num[n].x <= 0.0f);
+        ly[n] = (sL[n].y >= 0.0f) || (num[n].y <= 0.0f);
+    }
+#pragma unroll
+    KH_EACH {
+        rK[n] = sel(lx[n], ly[n], L[n][0], R[n][0]); pKd[n] = sel(lx[n], ly[n], L[n][1], R[n][1]);
+        uK[n] = sel(lx[n], ly[n], L[n][2], R[n][2]); vK[n] = sel(lx[n], ly[n], L[n][3], R[n][3]);
+        wK[n] = sel(lx[n], ly[n], L[n][4], R[n][4]); dsK[n] = sel(lx[n], ly[n], dsL[n], dsR[n]);
+        mK[n] = sel(lx[n], ly[n], mL[n], mR[n]);
+    }
+#pragma unroll
+    KH_EACH { pK[n] = add2(pKd[n], pref); sK[n] = add2(uK[n], dsK[n]); }
+#pragma unroll
+    KH_EACH {
+        ox[n] = (lx[n] ? sK[n].x : -sK[n].x) >= 0.0f;
+        oy[n] = (ly[n] ? sK[n].y : -sK[n].y) >= 0.0f;
+        D[n] = fma2(sK[n], den[n], neg2(num[n]));
+    }
+#pragma unroll
+    KH_EACH r[n] = rcp2(mul2(den[n], D[n]));
+#pragma unroll
+    KH_EACH { sst[n] = mul2(num[n], mul2(D[n], r[n])); inv[n] = mul2(den[n], mul2(den[n], r[n])); }
+#pragma unroll
+    KH_EACH {
+        ke[n] = fma2(wK[n], wK[n], fma2(vK[n], vK[n], mul2(uK[n], uK[n])));
+        EK[n] = fma2(pK[n], bc(g.igm1), mul2(mul2(bc(0.5f), rK[n]), ke[n]));
+    }
+#pragma unroll
+    KH_EACH { phi[n] = mul2(sst[n], inv[n]); pstKd[n] = fma2(mK[n], sub2(sst[n], uK[n]), pKd[n]); }
+#pragma unroll
+    KH_EACH { F0[n] = mul2(phi[n], mK[n]); A4[n] = fma2(EK[n], dsK[n], neg2(mul2(pK[n], uK[n]))); }
+#pragma unroll
+    KH_EACH {
+        F1[n] = fma2(F0[n], sst[n], pstKd[n]);
+        F4[n] = mul2(sst[n], fma2(A4[n], inv[n], mul2(add2(pstKd[n], pref), add2(one, phi[n]))));
+    }
+#pragma unroll
+    KH_EACH { G0[n] = mul2(rK[n], uK[n]); G4[n] = mul2(add2(EK[n], pK[n]), uK[n]); }
+#pragma unroll
+    KH_EACH G1[n] = fma2(G0[n], uK[n], pKd[n]);
+#pragma unroll
+    KH_EACH {
+        F0[n] = sel(ox[n], oy[n], G0[n], F0[n]);
+        F1[n] = sel(ox[n], oy[n], G1[n], F1[n]);
+        F4[n] = sel(ox[n], oy[n], G4[n], F4[n]);
+    }
+#pragma unroll
+    KH_EACH {
+        F[n][0] = F0[n]; F[n][1] = F1[n]; F[n][2] = mul2(F0[n], vK[n]); F[n][3] = mul2(F0[n], wK[n]); F[n][4] = F4[n];
+    }
+#undef KH_EACH
+}
+
+// states in the global frame (rho, p - pref, vx, vy, vz) -> face-normal frame of axis DIR, and the flux back
+template <int DIR>
+__device__ __forceinline__ void to_normal(const f2 q[5], f2 o[5])
+{
+    constexpr int iu = 2 + DIR, iv = 2 + (DIR + 1) % 3, iw = 2 + (DIR + 2) % 3;
+    o[0] = q[0]; o[1] = q[1]; o[2] = q[iu]; o[3] = q[iv]; o[4] = q[iw];
+}
+template <int DIR>
+__device__ __forceinline__ void from_normal(const f2 F[5], f2 Fo[5])
+{
+    constexpr int iu = 2 + DIR, iv = 2 + (DIR + 1) % 3, iw = 2 + (DIR + 2) % 3;
+    Fo[0] = F[0]; Fo[iu - 1] = F[1]; Fo[iv - 1] = F[2]; Fo[iw - 1] = F[3]; Fo[4] = F[4];
+}
+
 // One Heun stage.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin + dt L(Uin))
 // (Uout aliases U0) and the CFL rate maximum of Uout.  3D only.
 template <int STAGE>
@@ -185,7 +304,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
     if (warp < PRP) {
         // ================================ main warps: cells (i, ja), (i, ja+1) ========================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 " KH_TMA_MAIN_REGS ";");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 " KH_TMA_STR(KH_TMA_MAIN_REGS) ";");
         const int w = warp;
         constexpr int RAWF = PTY * PTX, RAWS = 5 * RAWF;              // double strides of raw / u0: field, slot
         constexpr int WTF = (PRP + 2) * (PTX + 4);                    // f2 field stride of Wt
@@ -244,7 +363,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
         for (int f = 0; f < 5; f++) { QRx[f] = QRy[f] = mk(0.f, 0.f); QLyo[f] = 0.f; dU[f] = make_double2(0.0, 0.0); }
 
-#pragma unroll 1
+#pragma unroll UNROLL
         for (int k = kfirst; k < kend; k++) {
             const bool live = k >= kbeg;
             // ---------------- phase A: x / y slopes of plane k from the tile ----------------
@@ -264,49 +383,54 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             }
             block_bar();
             // ---------------- phase B: fluxes of plane k, tile of plane k+1 ----------------
+            // The z, x and y Riemann problems of the pair are independent: they are solved in lock step
+            // (hllc2n).  In the priming iteration the x / y inputs are not valid yet; those results are
+            // computed all the same (one basic block) and never used.
             f2 Wn[5];
             double2 Fzhi[5];
             {
                 convert(k + 2, s_conv, par_conv, Wn, k + 2 < kend);
-                f2 qL[5], qR[5], F[5];
+                f2 L[3][5], R[3][5], Fn[3][5], F[5];
+                {
+                    f2 qL[5], qR[5];
 #pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    qL[f] = QLz[f];
-                    plm(Wa[f], Wb[f], Wn[f], QLz[f], qR[f]);
+                    for (int f = 0; f < 5; f++) {
+                        qL[f] = QLz[f];
+                        plm(Wa[f], Wb[f], Wn[f], QLz[f], qR[f]);
+                    }
+                    to_normal<2>(qL, L[0]);
+                    to_normal<2>(qR, R[0]);
+#pragma unroll
+                    for (int f = 0; f < 5; f++) qL[f] = qlx[f * QXF];
+                    to_normal<0>(qL, L[1]);
+                    to_normal<0>(QRx, R[1]);
+#pragma unroll
+                    for (int f = 0; f < 5; f++) qL[f] = mk(qly[f * QYF], QLyo[f]);
+                    to_normal<1>(qL, L[2]);
+                    to_normal<1>(QRy, R[2]);
                 }
-                face_flux2<2>(qL, qR, gas, F);
+                hllc2n<3>(L, R, gas, Fn);
+                from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     Fzhi[f] = make_double2(dtdz * (double)F[f].x, dtdz * (double)F[f].y);
                     dU[f] = make_double2(Fzlo[f].x - Fzhi[f].x, Fzlo[f].y - Fzhi[f].y);
                 }
-            }
-            if (live) {
-                {
-                    f2 qL[5], F[5];
+                from_normal<0>(Fn[1], F);
 #pragma unroll
-                    for (int f = 0; f < 5; f++) qL[f] = qlx[f * QXF];
-                    face_flux2<0>(qL, QRx, gas, F);
-#pragma unroll
-                    for (int f = 0; f < 5; f++) {
-                        const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
-                        fxs[f * QXF] = fd;
-                        dU[f].x = fma(dtdx, fd.x, dU[f].x);
-                        dU[f].y = fma(dtdx, fd.y, dU[f].y);
-                    }
+                for (int f = 0; f < 5; f++) {
+                    const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
+                    fxs[f * QXF] = fd;
+                    dU[f].x = fma(dtdx, fd.x, dU[f].x);
+                    dU[f].y = fma(dtdx, fd.y, dU[f].y);
                 }
-                {
-                    f2 qL[5], F[5];
+                from_normal<1>(Fn[2], F);
 #pragma unroll
-                    for (int f = 0; f < 5; f++) qL[f] = mk(qly[f * QYF], QLyo[f]);
-                    face_flux2<1>(qL, QRy, gas, F);
-#pragma unroll
-                    for (int f = 0; f < 5; f++) {
-                        const double flo = (double)F[f].x, fin = (double)F[f].y;
-                        fys[f * QYF] = flo;
-                        dU[f].x = fma(dtdy, flo - fin, dU[f].x);
-                        dU[f].y = fma(dtdy, fin, dU[f].y);
-                    }
+                for (int f = 0; f < 5; f++) {
+                    const double flo = (double)F[f].x, fin = (double)F[f].y;
+                    fys[f * QYF] = flo;
+                    dU[f].x = fma(dtdy, flo - fin, dU[f].x);
+                    dU[f].y = fma(dtdy, fin, dU[f].y);
                 }
             }
             if (k + 1 < kend) {
@@ -352,7 +476,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         }
         block_bar();  // the producer ships the last plane after this barrier
     } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 " KH_TMA_HALO_REGS ";");
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 " KH_TMA_STR(KH_TMA_HALO_REGS) ";");
     if (warp == WARP_HALO_Y) {
         // ================================ halo rows -2, -1, PTY, PTY+1 (lane = column) ==================
         const HaloSide lo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
