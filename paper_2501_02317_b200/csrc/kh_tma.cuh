@@ -35,6 +35,12 @@ using pr::face_flux2;
 using pr::recover;
 using pr::Gas;
 
+#ifndef KH_TMA_A_SPLIT
+#define KH_TMA_A_SPLIT 1   // phase A: all shared-memory loads, then the slopes, then all stores
+#endif
+#ifndef KH_TMA_C_SPLIT
+#define KH_TMA_C_SPLIT 1   // phase C: likewise
+#endif
 #ifndef KH_TMA_UNROLL
 #define KH_TMA_UNROLL 2
 #endif
@@ -367,6 +373,31 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         for (int k = kfirst; k < kend; k++) {
             const bool live = k >= kbeg;
             // ---------------- phase A: x / y slopes of plane k from the tile ----------------
+            // (all shared-memory loads first, all stores last: the compiler cannot reorder them itself)
+#if KH_TMA_A_SPLIT
+            if (live) {
+                f2 xm[5], xp[5], below[5], above[5], qLx[5], qLy[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    xm[f] = wt[f * WTF - 1];
+                    xp[f] = wt[f * WTF + 1];
+                    below[f] = wt[f * WTF - (PTX + 4)];
+                    above[f] = wt[f * WTF + (PTX + 4)];
+                }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const f2 q = Wa[f];
+                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
+                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
+                    QLyo[f] = qLy[f].x;
+                }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    qlx[f * QXF + 1] = qLx[f];
+                    qly[f * QYF + PTX] = qLy[f].y;
+                }
+            }
+#else
             if (live) {
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
@@ -381,6 +412,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     qly[f * QYF + PTX] = qLy.y;
                 }
             }
+#endif
             block_bar();
             // ---------------- phase B: fluxes of plane k, tile of plane k+1 ----------------
             // The z, x and y Riemann problems of the pair are independent: they are solved in lock step
@@ -413,24 +445,24 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    Fzhi[f] = make_double2(dtdz * (double)F[f].x, dtdz * (double)F[f].y);
-                    dU[f] = make_double2(Fzlo[f].x - Fzhi[f].x, Fzlo[f].y - Fzhi[f].y);
+                    Fzhi[f] = make_double2(__dmul_rn(dtdz, (double)F[f].x), __dmul_rn(dtdz, (double)F[f].y));
+                    dU[f] = make_double2(__dadd_rn(Fzlo[f].x, -Fzhi[f].x), __dadd_rn(Fzlo[f].y, -Fzhi[f].y));
                 }
                 from_normal<0>(Fn[1], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
                     fxs[f * QXF] = fd;
-                    dU[f].x = fma(dtdx, fd.x, dU[f].x);
-                    dU[f].y = fma(dtdx, fd.y, dU[f].y);
+                    dU[f].x = __fma_rn(dtdx, fd.x, dU[f].x);
+                    dU[f].y = __fma_rn(dtdx, fd.y, dU[f].y);
                 }
                 from_normal<1>(Fn[2], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     const double flo = (double)F[f].x, fin = (double)F[f].y;
                     fys[f * QYF] = flo;
-                    dU[f].x = fma(dtdy, flo - fin, dU[f].x);
-                    dU[f].y = fma(dtdy, fin, dU[f].y);
+                    dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin), dU[f].x);
+                    dU[f].y = __fma_rn(dtdy, fin, dU[f].y);
                 }
             }
             if (k + 1 < kend) {
@@ -439,33 +471,76 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             }
             block_bar();
             // ---------------- phase C: fp64 update of plane k, in place ----------------
+            // Loads first, stores last; explicitly rounded, so that the result does not depend on what the
+            // compiler contracts.
             if (live) {
                 double* su = raw0 + s_upd * RAWS;
                 const double* s0 = u00 + ((k - kbeg) & 1) * RAWS;
+                double2 fxh[5];
+                double fyh[5], ua[5], ub[5], va[5], vb[5];
                 if (STAGE == 2) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
-                double ua[5], ub[5];
+#if KH_TMA_C_SPLIT
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double2 fxh = fxs[f * QXF + 1];
-                    const double fyh = fys[f * QYF + PTX];
-                    double xa = su[f * RAWF] + fma(-dtdx, fxh.x, dU[f].x);
-                    double xb = su[f * RAWF + PTX] + fma(-dtdy, fyh, fma(-dtdx, fxh.y, dU[f].y));
+                    fxh[f] = fxs[f * QXF + 1];
+                    fyh[f] = fys[f * QYF + PTX];
+                    ua[f] = su[f * RAWF];
+                    ub[f] = su[f * RAWF + PTX];
+                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
+                }
+#endif
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+#if !KH_TMA_C_SPLIT
+                    fxh[f] = fxs[f * QXF + 1];
+                    fyh[f] = fys[f * QYF + PTX];
+                    ua[f] = su[f * RAWF];
+                    ub[f] = su[f * RAWF + PTX];
+                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
+#endif
+                    double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, fxh[f].x, dU[f].x));
+                    double xb = __dadd_rn(ub[f], __fma_rn(-dtdy, fyh[f], __fma_rn(-dtdx, fxh[f].y, dU[f].y)));
                     if (STAGE == 2) {
-                        xa = 0.5 * s0[f * RAWF] + 0.5 * xa;
-                        xb = 0.5 * s0[f * RAWF + PTX] + 0.5 * xb;
+                        xa = __fma_rn(0.5, va[f], __dmul_rn(0.5, xa));
+                        xb = __fma_rn(0.5, vb[f], __dmul_rn(0.5, xb));
                     }
                     ua[f] = xa;
                     ub[f] = xb;
+#if !KH_TMA_C_SPLIT
                     su[f * RAWF] = xa;
                     su[f * RAWF + PTX] = xb;
+#endif
                 }
+#if KH_TMA_C_SPLIT
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    su[f * RAWF] = ua[f];
+                    su[f * RAWF + PTX] = ub[f];
+                }
+#endif
                 fence_async_smem();  // the producer ships this box after the next barrier
-                if (STAGE == 2) {
-                    float ra = cfl_rate_from_cons<float>(ua, cc);
-                    float rb = cfl_rate_from_cons<float>(ub, cc);
-                    if (!(ra == ra)) ra = __int_as_float(0x7f800000);
-                    if (!(rb == rb)) rb = __int_as_float(0x7f800000);
-                    rate = mk(fmaxf(rate.x, ra), fmaxf(rate.y, rb));
+                if (STAGE == 2) {  // CFL rate of the new state (readings S1/S7), both cells at once
+                    using namespace pr;
+                    const float rfl = (float)KH_RHO_FLOOR, pfl = (float)KH_P_FLOOR;
+                    f2 r = mk((float)ua[0], (float)ub[0]);
+                    r = mk(r.x < rfl ? rfl : r.x, r.y < rfl ? rfl : r.y);  // comparisons, not fmax: a NaN must survive
+                    const f2 ir = rcp2(r);
+                    const f2 vx = mul2(mk((float)ua[1], (float)ub[1]), ir);
+                    const f2 vy = mul2(mk((float)ua[2], (float)ub[2]), ir);
+                    const f2 vz = mul2(mk((float)ua[3], (float)ub[3]), ir);
+                    const f2 v2 = fma2(vz, vz, fma2(vy, vy, mul2(vx, vx)));
+                    f2 p = mul2(bc(cc.gm1), fma2(mul2(bc(-0.5f), r), v2, mk((float)ua[4], (float)ub[4])));
+                    p = mk(p.x < pfl ? pfl : p.x, p.y < pfl ? pfl : p.y);
+                    const f2 gp = mul2(bc(cc.gamma), p);
+                    const f2 c = mul2(gp, rsqrt2(mul2(gp, r)));
+                    const f2 ax = mk(fabsf(vx.x), fabsf(vx.y)), ay = mk(fabsf(vy.x), fabsf(vy.y)),
+                             az = mk(fabsf(vz.x), fabsf(vz.y));
+                    f2 rt = mul2(add2(ax, c), bc(cc.idx));
+                    rt = fma2(add2(ay, c), bc(cc.idy), rt);
+                    rt = fma2(add2(az, c), bc(cc.idz), rt);
+                    if (!(rt.x == rt.x)) rt.x = __int_as_float(0x7f800000);
+                    if (!(rt.y == rt.y)) rt.y = __int_as_float(0x7f800000);
+                    rate = mk(fmaxf(rate.x, rt.x), fmaxf(rate.y, rt.y));
                 }
             }
             // rotate the z march and the ring
