@@ -126,8 +126,8 @@ int auto_variant(const kratos_hydro* h)
 int pick_zchunk(const kratos_hydro* h)
 {
     if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
-    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES || h->variant == KRATOS_KERNEL_TMA)
-               ? pr::auto_zchunk(h->g)
+    if (h->variant == KRATOS_KERNEL_TMA) return tma::auto_zchunk(h->g);
+    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES) ? pr::auto_zchunk(h->g)
                                                                                       : tiled_auto_zchunk(h->g);
 }
 

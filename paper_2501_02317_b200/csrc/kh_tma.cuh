@@ -16,10 +16,11 @@
 // (periodic wrap, clamp, mirror) made once per block plus the normal-velocity rule applied at conversion.
 //
 // Phases per plane k (as in kh_pair.cuh):
-//   A) x/y slopes from the primitive tile, left states published            | barrier 1
+//                                                                            | barrier 1
 //      [producer: store plane k-1, then refill its slot with plane k-1+NSLOT; halo plane k+3; U0(k+1)]
 //   B) z/x/y fluxes of plane k, conversion of plane k+2, tile of plane k+1   | barrier 2
 //   C) fp64 update of plane k, written in place; Heun average and CFL rate (stage 2)
+//   A) of plane k+1, fused with C: x/y slopes from the primitive tile, left states published
 #pragma once
 #include <cuda.h>
 
@@ -35,25 +36,23 @@ using pr::face_flux2;
 using pr::recover;
 using pr::Gas;
 
-#ifndef KH_TMA_A_SPLIT
-#define KH_TMA_A_SPLIT 1   // phase A: all shared-memory loads, then the slopes, then all stores
-#endif
-#ifndef KH_TMA_C_SPLIT
-#define KH_TMA_C_SPLIT 1   // phase C: likewise
-#endif
 #ifndef KH_TMA_UNROLL
 #define KH_TMA_UNROLL 2
 #endif
 constexpr int PTX = pr::PTX;       // 32
-constexpr int PTY = pr::PTY;       // 16
-constexpr int PRP = pr::PRP;       // 8 row pairs = main warps
+#ifndef KH_TMA_PTY
+#define KH_TMA_PTY 16              // tile height: 16 (one block per SM) or 8 (two blocks per SM)
+#endif
+constexpr int PTY = KH_TMA_PTY;
+constexpr int PRP = PTY / 2;       // row pairs = main warps (one or two warpgroups)
+constexpr int BLOCKS_PER_SM = 16 / PTY;
+static_assert(PTY == 16 || PTY == 8, "setmaxnreg acts on warpgroups: 4 or 8 main warps");
 constexpr int WARP_HALO_Y = PRP;
 constexpr int WARP_HALO_X = PRP + 1;
 constexpr int WARP_PRODUCER = PRP + 2;
 constexpr int NWARPS = PRP + 4;        // two main warpgroups + one auxiliary warpgroup (halo y, halo x, producer, idle):
                                        // setmaxnreg acts on whole warpgroups
 constexpr int NTHREADS = NWARPS * 32;
-constexpr int NHALO = 3;           // halo ring depth
 constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (register rotation becomes renaming)
 // register split of the three warpgroups (setmaxnreg): per scheduler 2 main warps + 1 auxiliary warp <= 16384
 #ifndef KH_TMA_MAIN_REGS
@@ -69,6 +68,7 @@ template <int STAGE>
 struct Cfg {
     static constexpr int NSLOT = (STAGE == 1) ? 5 : 4;   // raw ring depth (stage 2 shares the space with U0)
     static constexpr int NU0 = (STAGE == 2) ? 2 : 0;
+    static constexpr int NHALO = (STAGE == 2 && BLOCKS_PER_SM == 2) ? 2 : 3;   // halo ring depth
 };
 
 constexpr int OWN_BYTES = 5 * PTY * PTX * 8;    // one tile box
@@ -78,6 +78,7 @@ constexpr int COL_BYTES = 5 * PTY * 2 * 8;      // one halo column pair
 template <int STAGE>
 struct Smem {
     static constexpr int NSLOT = Cfg<STAGE>::NSLOT;
+    static constexpr int NHALO = Cfg<STAGE>::NHALO;
     alignas(128) double raw[NSLOT][5][PTY][PTX];              // fp64 state of the tile, planes in flight
     alignas(128) double u0[(STAGE == 2) ? 2 : 1][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
     alignas(128) double hrow[NHALO][2][5][2][PTX];            // halo rows: [lo/hi][field][box row][column]
@@ -271,11 +272,12 @@ __device__ __forceinline__ void from_normal(const f2 F[5], f2 Fo[5])
 // One Heun stage.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin + dt L(Uin))
 // (Uout aliases U0) and the CFL rate maximum of Uout.  3D only.
 template <int STAGE>
-__global__ void __launch_bounds__(NTHREADS, 1)
+__global__ void __launch_bounds__(NTHREADS, BLOCKS_PER_SM)
 stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
     using S = Smem<STAGE>;
     constexpr int NSLOT = S::NSLOT;
+    constexpr int NHALO = S::NHALO;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
@@ -372,47 +374,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll UNROLL
         for (int k = kfirst; k < kend; k++) {
             const bool live = k >= kbeg;
-            // ---------------- phase A: x / y slopes of plane k from the tile ----------------
-            // (all shared-memory loads first, all stores last: the compiler cannot reorder them itself)
-#if KH_TMA_A_SPLIT
-            if (live) {
-                f2 xm[5], xp[5], below[5], above[5], qLx[5], qLy[5];
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    xm[f] = wt[f * WTF - 1];
-                    xp[f] = wt[f * WTF + 1];
-                    below[f] = wt[f * WTF - (PTX + 4)];
-                    above[f] = wt[f * WTF + (PTX + 4)];
-                }
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    const f2 q = Wa[f];
-                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
-                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
-                    QLyo[f] = qLy[f].x;
-                }
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    qlx[f * QXF + 1] = qLx[f];
-                    qly[f * QYF + PTX] = qLy[f].y;
-                }
-            }
-#else
-            if (live) {
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    const f2 q = Wa[f];
-                    f2 qL;
-                    plm(wt[f * WTF - 1], q, wt[f * WTF + 1], qL, QRx[f]);
-                    qlx[f * QXF + 1] = qL;
-                    const f2 below = wt[f * WTF - (PTX + 4)], above = wt[f * WTF + (PTX + 4)];
-                    f2 qLy;
-                    plm(mk(below.y, q.x), q, mk(q.y, above.x), qLy, QRy[f]);
-                    QLyo[f] = qLy.x;
-                    qly[f * QYF + PTX] = qLy.y;
-                }
-            }
-#endif
             block_bar();
             // ---------------- phase B: fluxes of plane k, tile of plane k+1 ----------------
             // The z, x and y Riemann problems of the pair are independent: they are solved in lock step
@@ -470,16 +431,21 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 for (int f = 0; f < 5; f++) wt[f * WTF] = Wb[f];
             }
             block_bar();
-            // ---------------- phase C: fp64 update of plane k, in place ----------------
-            // Loads first, stores last; explicitly rounded, so that the result does not depend on what the
-            // compiler contracts.
-            if (live) {
+            // ---------------- phase C of plane k + phase A of plane k+1, as one block of straight-line code ----------
+            // C: fp64 update of plane k, written in place, explicitly rounded so that the result
+            //    does not depend on what the compiler contracts.
+            // A: x / y slopes of plane k+1 from the tile written in phase B, left states published for phase B(k+1).
+            // The two are independent; all shared-memory loads come first and all stores last (the compiler cannot
+            // reorder them itself), so that their latencies overlap.  In the priming iteration C works on stale
+            // data and in the last iteration A does: both results are never used (the in-place write then lands in
+            // a slot whose plane has been converted already and is refilled later).
+            {
                 double* su = raw0 + s_upd * RAWS;
                 const double* s0 = u00 + ((k - kbeg) & 1) * RAWS;
+                if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
                 double2 fxh[5];
                 double fyh[5], ua[5], ub[5], va[5], vb[5];
-                if (STAGE == 2) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
-#if KH_TMA_C_SPLIT
+                f2 xm[5], xp[5], below[5], above[5], qLx[5], qLy[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     fxh[f] = fxs[f * QXF + 1];
@@ -488,16 +454,15 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     ub[f] = su[f * RAWF + PTX];
                     if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
                 }
-#endif
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-#if !KH_TMA_C_SPLIT
-                    fxh[f] = fxs[f * QXF + 1];
-                    fyh[f] = fys[f * QYF + PTX];
-                    ua[f] = su[f * RAWF];
-                    ub[f] = su[f * RAWF + PTX];
-                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
-#endif
+                    xm[f] = wt[f * WTF - 1];
+                    xp[f] = wt[f * WTF + 1];
+                    below[f] = wt[f * WTF - (PTX + 4)];
+                    above[f] = wt[f * WTF + (PTX + 4)];
+                }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
                     double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, fxh[f].x, dU[f].x));
                     double xb = __dadd_rn(ub[f], __fma_rn(-dtdy, fyh[f], __fma_rn(-dtdx, fxh[f].y, dU[f].y)));
                     if (STAGE == 2) {
@@ -506,20 +471,23 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     }
                     ua[f] = xa;
                     ub[f] = xb;
-#if !KH_TMA_C_SPLIT
-                    su[f * RAWF] = xa;
-                    su[f * RAWF + PTX] = xb;
-#endif
                 }
-#if KH_TMA_C_SPLIT
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const f2 q = Wb[f];  // W(k+1)
+                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
+                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
+                    QLyo[f] = qLy[f].x;
+                }
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     su[f * RAWF] = ua[f];
                     su[f * RAWF + PTX] = ub[f];
+                    qlx[f * QXF + 1] = qLx[f];
+                    qly[f * QYF + PTX] = qLy[f].y;
                 }
-#endif
-                fence_async_smem();  // the producer ships this box after the next barrier
-                if (STAGE == 2) {  // CFL rate of the new state (readings S1/S7), both cells at once
+                fence_async_smem();  // the producer ships the updated box after the next barrier
+                if (STAGE == 2 && live) {  // CFL rate of the new state (readings S1/S7), both cells at once
                     using namespace pr;
                     const float rfl = (float)KH_RHO_FLOOR, pfl = (float)KH_P_FLOOR;
                     f2 r = mk((float)ua[0], (float)ub[0]);
@@ -623,7 +591,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         block_bar();
     } else if (warp == WARP_HALO_X) {
         // ================================ halo columns -2, -1, PTX, PTX+1 =============================
-        const int cid = lane & 3, rp = lane >> 2;                   // column id, row pair
+        const int cid = lane & 3, rp = min(lane >> 2, PRP - 1);     // column id, row pair
+        const bool xact = (lane >> 2) < PRP;                        // (a tile of 8 rows keeps half the lanes busy)
         const int col = (cid < 2) ? cid - 2 : PTX + cid - 2;
         const HaloSide side = (cid < 2) ? halo_side(i0 - 2, nx, g.bc[0], g.bc[1]) : halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
         const int bidx = (cid & 1) ? side.idx1 : side.idx0;
@@ -647,13 +616,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 for (int f = 0; f < 5; f++) {
                     f2 qL, qR;
                     plm(wt[f * WTF + dl], W[f], wt[f * WTF + dr], qL, qR);
-                    if (cid == 1) sm.QLx[f][rp][0] = qL;   // column -1: left state of the tile's low x face
-                    if (cid == 2) sm.QRxR[f][rp] = qR;     // column PTX: right state of the tile's high x face
+                    if (cid == 1 && xact) sm.QLx[f][rp][0] = qL;   // column -1: left state of the tile's low x face
+                    if (cid == 2 && xact) sm.QRxR[f][rp] = qR;     // column PTX: right state of the tile's high x face
                 }
             }
             block_bar();
             // phase B: flux through the tile's high x face of plane k; halo columns of plane k+1
-            if (live && cid == 2) {
+            if (live && cid == 2 && xact) {
                 f2 qL[5], qR[5], F[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) { qL[f] = sm.QLx[f][rp][PTX]; qR[f] = sm.QRxR[f][rp]; }
@@ -673,7 +642,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     W[f] = mk(Wa[f], Wb[f]);
-                    wt[f * WTF] = W[f];
+                    if (xact) wt[f * WTF] = W[f];
                 }
                 if (++hs == NHALO) { hs = 0; hpar ^= 1u; }
             }
@@ -819,11 +788,19 @@ inline void build_maps(StageMaps* sm, const double* A, const double* B, const Gr
     sm->ok = true;
 }
 
-inline int auto_zchunk(const Grid& g) { return pr::auto_zchunk(g); }
+inline int auto_zchunk(const Grid& g)
+{
+    // >= ~12 waves of thread blocks over the 148 SMs, slabs of >= 32 planes
+    const long long tiles = (long long)(g.n[0] / PTX) * (g.n[1] / PTY);
+    int chunk = g.n[2];
+    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * BLOCKS_PER_SM * 12) chunk = (chunk + 1) / 2;
+    return chunk;
+}
 
 inline void configure()
 {
-    static_assert(sizeof(Smem<1>) + 128 <= 227 * 1024 && sizeof(Smem<2>) + 128 <= 227 * 1024,
+    constexpr size_t per_block = (228 * 1024) / BLOCKS_PER_SM - 1024;
+    static_assert(sizeof(Smem<1>) + 128 <= per_block && sizeof(Smem<2>) + 128 <= per_block,
                   "tile does not fit the shared memory of one SM");
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
