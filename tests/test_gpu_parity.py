@@ -376,3 +376,49 @@ def test_step_rejects_bad_dt_and_nonfinite_state_is_reported():
         h.cfl_dt(0.4)
     assert ei.value.code == binding.ERR_NONFINITE
     h.destroy()
+
+
+# --------------------------------------------------------------------------- full size, the launch configuration bench.py times
+def test_c5_full_size_sampled_against_oracle():
+    """C5 at BASELINE.json's size (512^3 periodic, mixed precision, auto kernel and slab height = what bench.py
+    times): two Heun steps on the GPU; sampled 12^3 sub-blocks are recomputed by the oracle from the initial
+    state of their domain of dependence (2 steps x 2 stages x 2 cells = 8 cells each side), with the same dt
+    sequence.  Conserved totals of the whole block must not drift."""
+    n, nstep, halo, core = 512, 2, 8, 12
+    try:
+        pr = inputs.turbulence_3d(n, seed=5, nsteps=nstep)
+    except MemoryError:
+        pytest.skip("not enough host memory for the 512^3 state")
+    h = make(pr, MIXED)
+    T0 = h.totals()
+    dts = []
+    for _ in range(nstep):
+        dts.append(h.cfl_dt(0.4))   # fp64 rate maximum over the whole block (matches the oracle's to 1e-13)
+        h.step(dts[-1])
+    T1 = h.totals()
+    Ug = h.get_state()
+    assert h.floor_hits() == 0
+    h.destroy()
+    A0 = np.array([float(np.abs(pr.U[m]).sum()) for m in range(5)])
+    assert (np.abs(T1 - T0) / np.maximum(np.abs(T0), A0)).max() <= 1e-13
+    # the first dt against the oracle's own reduction over the full state
+    assert dts[0] == pytest.approx(oracle.cfl_dt(pr.U, pr.gamma, 0.4), rel=1e-13)
+    rng = np.random.default_rng(123)
+    w = core + 2 * halo
+    corners = [(0, 0, 0), (n - core, n - core, n - core), (250, 9, 121)]   # tile / slab seams and the periodic wrap
+    corners += [tuple(int(c) for c in rng.integers(0, n, 3)) for _ in range(5)]
+    for (k0, j0, i0) in corners:
+        kk = (np.arange(k0 - halo, k0 - halo + w)) % n
+        jj = (np.arange(j0 - halo, j0 - halo + w)) % n
+        ii = (np.arange(i0 - halo, i0 - halo + w)) % n
+        sub = np.ascontiguousarray(pr.U[:, kk][:, :, jj][:, :, :, ii])
+        for dt in dts:
+            # free boundaries on the sub-block: wrong only within 4 cells of its faces per step
+            oracle.step(sub, pr.gamma, (F,) * 6, dt, spacing=(1.0 / n,) * 3)
+        ref = sub[:, halo:halo + core, halo:halo + core, halo:halo + core]
+        kc = (np.arange(k0, k0 + core)) % n
+        jc = (np.arange(j0, j0 + core)) % n
+        ic = (np.arange(i0, i0 + core)) % n
+        got = Ug[:, kc][:, :, jc][:, :, :, ic]
+        err = rel_l1_fields(got, ref)
+        assert max(err) <= TOL[MIXED], ((k0, j0, i0), err)
