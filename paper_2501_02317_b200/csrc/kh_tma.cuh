@@ -36,6 +36,11 @@ using pr::face_flux2;
 using pr::recover;
 using pr::Gas;
 
+#ifdef KH_WHATIF_NOF2F   // timing experiment only (wrong results): no fp32 -> fp64 conversion instructions
+#define KH_CVT(x) __hiloint2double(__float_as_int(x), 0)
+#else
+#define KH_CVT(x) ((double)(x))
+#endif
 #ifndef KH_TMA_UNROLL
 #define KH_TMA_UNROLL 2
 #endif
@@ -50,7 +55,8 @@ static_assert(PTY == 16 || PTY == 8, "setmaxnreg acts on warpgroups: 4 or 8 main
 constexpr int WARP_HALO_Y = PRP;
 constexpr int WARP_HALO_X = PRP + 1;
 constexpr int WARP_PRODUCER = PRP + 2;
-constexpr int NWARPS = PRP + 4;        // two main warpgroups + one auxiliary warpgroup (halo y, halo x, producer, idle):
+constexpr int WARP_HALO_Y2 = PRP + 3;
+constexpr int NWARPS = PRP + 4;        // main warpgroup(s) + one auxiliary warpgroup (halo rows low, halo columns, producer, halo rows high):
                                        // setmaxnreg acts on whole warpgroups
 constexpr int NTHREADS = NWARPS * 32;
 constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (register rotation becomes renaming)
@@ -139,7 +145,23 @@ __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commi
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+#ifdef KH_TMA_TIMING   // working instrumentation: cycles spent computing / waiting at the block barrier, per warp
+struct BarTimer { long long t_last, work[2], wait[2]; int n; unsigned addr; };
+__device__ __forceinline__ void block_bar_t(BarTimer& bt)
+{
+    long long t0, t1;
+    unsigned x;
+    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t0)::"memory");
+    asm volatile("bar.sync 0;" ::: "memory");
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(x) : "r"(bt.addr) : "memory");  // blocks until the barrier opens
+    if (x == 0xdeadbeefu) bt.n += 1000;                                                      // (in-order issue: consumes x)
+    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1)::"memory");
+    bt.work[bt.n & 1] += t0 - bt.t_last; bt.wait[bt.n & 1] += t1 - t0; bt.t_last = t1; bt.n++;
+}
+#define block_bar() block_bar_t(bt)
+#else
 __device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "memory"); }
+#endif
 
 // Where the two halo cells beyond one side of the tile come from (Sec. 3.1.1): first source coordinate of the
 // 2-wide box, the position inside the box of each of the two cells, and the normal-velocity rule.
@@ -309,6 +331,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
     int hits = 0;
     f2 rate = mk(0.0f, 0.0f);
+#ifdef KH_TMA_TIMING
+    BarTimer bt; bt.t_last = clock64(); bt.work[0] = bt.work[1] = bt.wait[0] = bt.wait[1] = 0; bt.n = 0; bt.addr = smem_u32(&sm.red[0]);
+#endif
 
     if (warp < PRP) {
         // ================================ main warps: cells (i, ja), (i, ja+1) ========================
@@ -406,13 +431,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    Fzhi[f] = make_double2(__dmul_rn(dtdz, (double)F[f].x), __dmul_rn(dtdz, (double)F[f].y));
+                    Fzhi[f] = make_double2(__dmul_rn(dtdz, KH_CVT(F[f].x)), __dmul_rn(dtdz, KH_CVT(F[f].y)));
                     dU[f] = make_double2(__dadd_rn(Fzlo[f].x, -Fzhi[f].x), __dadd_rn(Fzlo[f].y, -Fzhi[f].y));
                 }
                 from_normal<0>(Fn[1], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
+                    const double2 fd = make_double2(KH_CVT(F[f].x), KH_CVT(F[f].y));
                     fxs[f * QXF] = fd;
                     dU[f].x = __fma_rn(dtdx, fd.x, dU[f].x);
                     dU[f].y = __fma_rn(dtdx, fd.y, dU[f].y);
@@ -420,7 +445,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<1>(Fn[2], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double flo = (double)F[f].x, fin = (double)F[f].y;
+                    const double flo = KH_CVT(F[f].x), fin = KH_CVT(F[f].y);
                     fys[f * QYF] = flo;
                     dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin), dU[f].x);
                     dU[f].y = __fma_rn(dtdy, fin, dU[f].y);
@@ -446,6 +471,17 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 double2 fxh[5];
                 double fyh[5], ua[5], ub[5], va[5], vb[5];
                 f2 xm[5], xp[5], below[5], above[5], qLx[5], qLy[5];
+#ifdef KH_WHATIF_LESS_SMEM   // timing experiment only (wrong results): 70 of ~230 shared-memory wavefronts per plane dropped
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    fxh[f] = make_double2(dU[f].y, dU[f].x);
+                    fyh[f] = dU[f].x;
+                    ua[f] = su[f * RAWF];
+                    ub[f] = su[f * RAWF + PTX];
+                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
+                    xm[f] = Wa[f]; xp[f] = Wn[f]; below[f] = Wn[f]; above[f] = Wa[f];
+                }
+#else
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     fxh[f] = fxs[f * QXF + 1];
@@ -461,6 +497,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     below[f] = wt[f * WTF - (PTX + 4)];
                     above[f] = wt[f * WTF + (PTX + 4)];
                 }
+#endif
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, fxh[f].x, dU[f].x));
@@ -472,22 +509,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     ua[f] = xa;
                     ub[f] = xb;
                 }
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    const f2 q = Wb[f];  // W(k+1)
-                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
-                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
-                    QLyo[f] = qLy[f].x;
-                }
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    su[f * RAWF] = ua[f];
-                    su[f * RAWF + PTX] = ub[f];
-                    qlx[f * QXF + 1] = qLx[f];
-                    qly[f * QYF + PTX] = qLy[f].y;
-                }
-                fence_async_smem();  // the producer ships the updated box after the next barrier
-                if (STAGE == 2 && live) {  // CFL rate of the new state (readings S1/S7), both cells at once
+                if (STAGE == 2) {  // CFL rate of the new state (readings S1/S7), both cells at once; no branch:
+                                   // the priming iteration computes it on stale data and drops it
                     using namespace pr;
                     const float rfl = (float)KH_RHO_FLOOR, pfl = (float)KH_P_FLOOR;
                     f2 r = mk((float)ua[0], (float)ub[0]);
@@ -508,8 +531,23 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     rt = fma2(add2(az, c), bc(cc.idz), rt);
                     if (!(rt.x == rt.x)) rt.x = __int_as_float(0x7f800000);
                     if (!(rt.y == rt.y)) rt.y = __int_as_float(0x7f800000);
-                    rate = mk(fmaxf(rate.x, rt.x), fmaxf(rate.y, rt.y));
+                    rate = mk(live ? fmaxf(rate.x, rt.x) : rate.x, live ? fmaxf(rate.y, rt.y) : rate.y);
                 }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    const f2 q = Wb[f];  // W(k+1)
+                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
+                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
+                    QLyo[f] = qLy[f].x;
+                }
+#pragma unroll
+                for (int f = 0; f < 5; f++) {
+                    su[f * RAWF] = ua[f];
+                    su[f * RAWF + PTX] = ub[f];
+                    qlx[f * QXF + 1] = qLx[f];
+                    qly[f * QYF + PTX] = qLy[f].y;
+                }
+                fence_async_smem();  // the producer ships the updated box after the next barrier
             }
             // rotate the z march and the ring
 #pragma unroll
@@ -520,70 +558,87 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         block_bar();  // the producer ships the last plane after this barrier
     } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 " KH_TMA_STR(KH_TMA_HALO_REGS) ";");
-    if (warp == WARP_HALO_Y) {
-        // ================================ halo rows -2, -1, PTY, PTY+1 (lane = column) ==================
-        const HaloSide lo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
-        const HaloSide hi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
+    if (warp == WARP_HALO_Y || warp == WARP_HALO_Y2) {
+        // ============ halo rows: warp HALO_Y owns rows -2, -1, warp HALO_Y2 rows PTY, PTY+1 (lane = column) ============
+        const bool top = (warp == WARP_HALO_Y2);
+        const HaloSide hsd = top ? halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]) : halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
         constexpr int HF = 2 * PTX, HSIDE = 5 * HF, HSLOT = 2 * HSIDE;   // double strides of hrow: field, side, slot
-        const int off[4] = {lo.idx0 * PTX + lane, lo.idx1 * PTX + lane, HSIDE + hi.idx0 * PTX + lane,
-                            HSIDE + hi.idx1 * PTX + lane};
-        const int ry[4] = {lo.rule, lo.rule, hi.rule, hi.rule};
+        const int off0 = (top ? HSIDE : 0) + hsd.idx0 * PTX + lane, off1 = (top ? HSIDE : 0) + hsd.idx1 * PTX + lane;
+        const int ry = hsd.rule;
         const double* const h0 = &sm.hrow[0][0][0][0][0];
         constexpr int WTF = (PRP + 2) * (PTX + 4);
         constexpr int QYF = (PRP + 1) * PTX;
-        f2* const wlo = &sm.Wt[0][0][lane + 2];          // rows -2, -1
-        f2* const whi = &sm.Wt[0][PRP + 1][lane + 2];    // rows PTY, PTY+1
-        float W[4][5];
+        f2* const wown = &sm.Wt[0][top ? PRP + 1 : 0][lane + 2];                 // the warp's own row pair of the tile
+        const f2* const wnext = wown + (top ? -(PTX + 4) : (PTX + 4));          // the tile's row pair next to it
+        float W0[5], W1[5];   // the two rows, low row first
 #pragma unroll
-        for (int r = 0; r < 4; r++)
-#pragma unroll
-            for (int f = 0; f < 5; f++) W[r][f] = 0.0f;
+        for (int f = 0; f < 5; f++) W0[f] = W1[f] = 0.0f;
         int hs = 0;
         unsigned hpar = 0u;
 #pragma unroll 1
         for (int k = kfirst; k < kend; k++) {
             const bool live = k >= kbeg;
-            // phase A: limited y states of rows -1 and PTY of plane k
+            // phase A: limited y state of the row next to the tile (row -1 resp. PTY) of plane k
             if (live) {
+                f2 nb[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) nb[f] = wnext[f * WTF];
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const f2 r01 = wlo[f * WTF + (PTX + 4)];        // rows 0, 1
-                    const f2 rtop = whi[f * WTF - (PTX + 4)];       // rows PTY-2, PTY-1
+                    // bottom: rows (-2, -1, 0) -> left state of the tile's low y face; top: rows (PTY-1, PTY, PTY+1)
+                    // -> right state of the tile's high y face
+                    const float qm = top ? nb[f].y : W0[f], q = top ? W0[f] : W1[f], qp = top ? W1[f] : nb[f].x;
                     f2 qL, qR;
-                    plm(mk(W[0][f], rtop.y), mk(W[1][f], W[2][f]), mk(r01.x, W[3][f]), qL, qR);
-                    sm.QLy[f][0][lane] = qL.x;    // row -1: left state of the tile's low y face
-                    sm.QRyT[f][lane] = qR.y;      // row PTY: right state of the tile's high y face
+                    plm(mk(qm, qm), mk(q, q), mk(qp, qp), qL, qR);
+                    if (top) sm.QRyT[f][lane] = qR.x;
+                    else     sm.QLy[f][0][lane] = qL.x;
                 }
             }
             block_bar();
-            // phase B: flux through the tile's high y face of plane k; halo rows of plane k+1
-            if (live) {
-                f2 qL[5], qR[5], F[5];
+            // phase B: (top) flux through the tile's high y face of plane k; halo rows of plane k+1
+            if (live && top) {
+                // One packed Riemann call for both high edges of the tile: component .x solves the y face above
+                // column `lane` (32 faces), component .y of lanes 0..PTY-1 the x face right of row `lane`.
+                const int xr = min(lane, PTY - 1);
+                const float* const qlx_e = reinterpret_cast<const float*>(&sm.QLx[0][xr >> 1][PTX]) + (xr & 1);
+                const float* const qrx_e = reinterpret_cast<const float*>(&sm.QRxR[0][xr >> 1]) + (xr & 1);
+                constexpr int QXF2 = 2 * PRP * (PTX + 1), QRF2 = 2 * PRP;   // float strides of QLx / QRxR per field
+                float yl[5], yr[5], xl[5], xrr[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const float l = sm.QLy[f][PRP][lane], r = sm.QRyT[f][lane];
-                    qL[f] = mk(l, l);
-                    qR[f] = mk(r, r);
+                    yl[f] = sm.QLy[f][PRP][lane];
+                    yr[f] = sm.QRyT[f][lane];
+                    xl[f] = qlx_e[f * QXF2];
+                    xrr[f] = qrx_e[f * QRF2];
                 }
-                face_flux2<1>(qL, qR, gas, F);
+                // face-normal frames: y face (rho, p, vy, vz, vx), x face (rho, p, vx, vy, vz)
+                const f2 L[5] = {mk(yl[0], xl[0]), mk(yl[1], xl[1]), mk(yl[3], xl[2]), mk(yl[4], xl[3]), mk(yl[2], xl[4])};
+                const f2 R[5] = {mk(yr[0], xrr[0]), mk(yr[1], xrr[1]), mk(yr[3], xrr[2]), mk(yr[4], xrr[3]), mk(yr[2], xrr[4])};
+                f2 F[5];
+                pr::hllc2(L, R, gas, F);
+                // back to conserved-field order: y face (F0, F4', F1, F3', F4) with normal momentum in slot 2
+                sm.Fy[0][PRP][lane] = (double)F[0].x;
+                sm.Fy[2][PRP][lane] = (double)F[1].x;
+                sm.Fy[3][PRP][lane] = (double)F[2].x;
+                sm.Fy[1][PRP][lane] = (double)F[3].x;
+                sm.Fy[4][PRP][lane] = (double)F[4].x;
+                if (lane < PTY) {
+                    double* const fxe = reinterpret_cast<double*>(&sm.Fx[0][lane >> 1][PTX]) + (lane & 1);
+                    constexpr int FXF2 = 2 * PRP * (PTX + 1);   // double stride of Fx per field
 #pragma unroll
-                for (int f = 0; f < 5; f++) sm.Fy[f][PRP][lane] = (double)F[f].x;
+                    for (int f = 0; f < 5; f++) fxe[f * FXF2] = (double)F[f].y;
+                }
             }
             if (k + 1 < kend) {
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = h0 + hs * HSLOT;
+                double u0[5], u1[5];
 #pragma unroll
-                for (int r = 0; r < 4; r++) {
-                    double u[5];
+                for (int f = 0; f < 5; f++) { u0[f] = s[off0 + f * HF]; u1[f] = s[off1 + f * HF]; }
+                (void)recover(u0[0], u0[1], u0[2], u0[3], u0[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W0);
+                (void)recover(u1[0], u1[1], u1[2], u1[3], u1[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W1);
 #pragma unroll
-                    for (int f = 0; f < 5; f++) u[f] = s[off[r] + f * HF];
-                    (void)recover(u[0], u[1], u[2], u[3], u[4], gm1, pref_d, VN_KEEP, ry[r], VN_KEEP, W[r]);
-                }
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    wlo[f * WTF] = mk(W[0][f], W[1][f]);
-                    whi[f * WTF] = mk(W[2][f], W[3][f]);
-                }
+                for (int f = 0; f < 5; f++) wown[f * WTF] = mk(W0[f], W1[f]);
                 if (++hs == NHALO) { hs = 0; hpar ^= 1u; }
             }
             block_bar();
@@ -612,24 +667,21 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             const bool live = k >= kbeg;
             // phase A: limited x states of columns -1 and PTX of plane k
             if (live) {
+                // loads first, stores last: the shared-memory pipe is busiest in this window and every load this warp
+                // waits for on its own is time the main warps spend at the barrier
+                f2 wl[5], wr[5], qL[5], qR[5];
+#pragma unroll
+                for (int f = 0; f < 5; f++) { wl[f] = wt[f * WTF + dl]; wr[f] = wt[f * WTF + dr]; }
+#pragma unroll
+                for (int f = 0; f < 5; f++) plm(wl[f], W[f], wr[f], qL[f], qR[f]);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    f2 qL, qR;
-                    plm(wt[f * WTF + dl], W[f], wt[f * WTF + dr], qL, qR);
-                    if (cid == 1 && xact) sm.QLx[f][rp][0] = qL;   // column -1: left state of the tile's low x face
-                    if (cid == 2 && xact) sm.QRxR[f][rp] = qR;     // column PTX: right state of the tile's high x face
+                    if (cid == 1 && xact) sm.QLx[f][rp][0] = qL[f];   // column -1: left state of the tile's low x face
+                    if (cid == 2 && xact) sm.QRxR[f][rp] = qR[f];     // column PTX: right state of the tile's high x face
                 }
             }
             block_bar();
-            // phase B: flux through the tile's high x face of plane k; halo columns of plane k+1
-            if (live && cid == 2 && xact) {
-                f2 qL[5], qR[5], F[5];
-#pragma unroll
-                for (int f = 0; f < 5; f++) { qL[f] = sm.QLx[f][rp][PTX]; qR[f] = sm.QRxR[f][rp]; }
-                face_flux2<0>(qL, qR, gas, F);
-#pragma unroll
-                for (int f = 0; f < 5; f++) sm.Fx[f][rp][PTX] = make_double2((double)F[f].x, (double)F[f].y);
-            }
+            // phase B: halo columns of plane k+1 (the flux through the tile's high x face is the producer warp's)
             if (k + 1 < kend) {
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = c0 + hs * CSLOT;
@@ -694,6 +746,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
                     tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
                 }
+            }
+            __syncwarp();
+            if (lane == 0) {  // refill the slot the store is reading from
+                const bool stored = k - 1 >= kbeg;
                 const int p = k - 1 + NSLOT;
                 if (p <= plast) {
                     if (stored) tma_wait_read0();  // the store has read the box: the slot may be refilled
@@ -713,14 +769,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             tma_wait_all0();
         }
         __syncwarp();
-    } else {
-        // the fourth warp of the auxiliary warpgroup only keeps the barriers
-#pragma unroll 1
-        for (int k = kfirst; k < kend; k++) { block_bar(); block_bar(); }
-        block_bar();
     }
     }
 
+#ifdef KH_TMA_TIMING
+    if (blockIdx.x == 3 && blockIdx.y == 5 && blockIdx.z == 1 && lane == 0)
+        printf("stage %d warp %2d: barriers %d | before bar1: work %lld wait %lld | before bar2: work %lld wait %lld\n", STAGE, warp, bt.n, bt.work[0], bt.wait[0], bt.work[1], bt.wait[1]);
+#endif
     if (hits) atomicAdd(&ctrl->floor_hits, (unsigned long long)hits);
     if (STAGE == 2) {
         __syncthreads();
