@@ -94,8 +94,8 @@ struct Smem {
     f2 QRxR[5][PRP];                                          // right state at x face PTX (from halo column PTX)
     float QLy[5][PRP + 1][PTX];                               // left states at y faces r = 0..PRP (from row 2r-1)
     float QRyT[5][PTX];                                       // right state at y face PRP (from halo row PTY)
-    double2 Fx[5][PRP][PTX + 1];                              // fp64 fluxes through x faces
-    double Fy[5][PRP + 1][PTX];                               // fp64 fluxes through the y faces between row pairs
+    f2 Fx[5][PRP][PTX + 1];                                   // float_t fluxes through x faces (each side converts: same bits)
+    float Fy[5][PRP + 1][PTX];                                // float_t fluxes through the y faces between row pairs
     double red[32];
     unsigned long long full_raw[NSLOT];
     unsigned long long full_halo[NHALO];
@@ -348,8 +348,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         f2* const wt = &sm.Wt[0][w + 1][lane + 2];
         f2* const qlx = &sm.QLx[0][w][lane];      // left state of the own low x face; own high face is + 1
         float* const qly = &sm.QLy[0][w][lane];   // left state of the pair's low y face; the pair's high face is + PTX
-        double2* const fxs = &sm.Fx[0][w][lane];
-        double* const fys = &sm.Fy[0][w][lane];
+        f2* const fxs = &sm.Fx[0][w][lane];
+        float* const fys = &sm.Fy[0][w][lane];
 
         const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1], dtdz = dt * g.inv_dx[2];
         const CflConst<float> cc(g);
@@ -438,7 +438,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     const double2 fd = make_double2(KH_CVT(F[f].x), KH_CVT(F[f].y));
-                    fxs[f * QXF] = fd;
+                    fxs[f * QXF] = F[f];
                     dU[f].x = __fma_rn(dtdx, fd.x, dU[f].x);
                     dU[f].y = __fma_rn(dtdx, fd.y, dU[f].y);
                 }
@@ -446,7 +446,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     const double flo = KH_CVT(F[f].x), fin = KH_CVT(F[f].y);
-                    fys[f * QYF] = flo;
+                    fys[f * QYF] = F[f].x;
                     dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin), dU[f].x);
                     dU[f].y = __fma_rn(dtdy, fin, dU[f].y);
                 }
@@ -468,20 +468,11 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 double* su = raw0 + s_upd * RAWS;
                 const double* s0 = u00 + ((k - kbeg) & 1) * RAWS;
                 if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
-                double2 fxh[5];
-                double fyh[5], ua[5], ub[5], va[5], vb[5];
-                f2 xm[5], xp[5], below[5], above[5], qLx[5], qLy[5];
-#ifdef KH_WHATIF_LESS_SMEM   // timing experiment only (wrong results): 70 of ~230 shared-memory wavefronts per plane dropped
-#pragma unroll
-                for (int f = 0; f < 5; f++) {
-                    fxh[f] = make_double2(dU[f].y, dU[f].x);
-                    fyh[f] = dU[f].x;
-                    ua[f] = su[f * RAWF];
-                    ub[f] = su[f * RAWF + PTX];
-                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
-                    xm[f] = Wa[f]; xp[f] = Wn[f]; below[f] = Wn[f]; above[f] = Wa[f];
-                }
-#else
+                f2 fxh[5];
+                float fyh[5];
+                double ua[5], ub[5], va[5], vb[5];
+                f2 xm[5], xp[5], qLx[5], qLy[5];
+                float below[5], above[5];   // rows 2w-1 and 2w+2: the near halves of the neighbouring row pairs
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     fxh[f] = fxs[f * QXF + 1];
@@ -494,14 +485,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 for (int f = 0; f < 5; f++) {
                     xm[f] = wt[f * WTF - 1];
                     xp[f] = wt[f * WTF + 1];
-                    below[f] = wt[f * WTF - (PTX + 4)];
-                    above[f] = wt[f * WTF + (PTX + 4)];
+                    below[f] = wt[f * WTF - (PTX + 4)].y;
+                    above[f] = wt[f * WTF + (PTX + 4)].x;
                 }
-#endif
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, fxh[f].x, dU[f].x));
-                    double xb = __dadd_rn(ub[f], __fma_rn(-dtdy, fyh[f], __fma_rn(-dtdx, fxh[f].y, dU[f].y)));
+                    double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, (double)fxh[f].x, dU[f].x));
+                    double xb = __dadd_rn(ub[f], __fma_rn(-dtdy, (double)fyh[f], __fma_rn(-dtdx, (double)fxh[f].y, dU[f].y)));
                     if (STAGE == 2) {
                         xa = __fma_rn(0.5, va[f], __dmul_rn(0.5, xa));
                         xb = __fma_rn(0.5, vb[f], __dmul_rn(0.5, xb));
@@ -537,7 +527,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 for (int f = 0; f < 5; f++) {
                     const f2 q = Wb[f];  // W(k+1)
                     plm(xm[f], q, xp[f], qLx[f], QRx[f]);
-                    plm(mk(below[f].y, q.x), q, mk(q.y, above[f].x), qLy[f], QRy[f]);
+                    plm(mk(below[f], q.x), q, mk(q.y, above[f]), qLy[f], QRy[f]);
                     QLyo[f] = qLy[f].x;
                 }
 #pragma unroll
@@ -617,16 +607,16 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 f2 F[5];
                 pr::hllc2(L, R, gas, F);
                 // back to conserved-field order: y face (F0, F4', F1, F3', F4) with normal momentum in slot 2
-                sm.Fy[0][PRP][lane] = (double)F[0].x;
-                sm.Fy[2][PRP][lane] = (double)F[1].x;
-                sm.Fy[3][PRP][lane] = (double)F[2].x;
-                sm.Fy[1][PRP][lane] = (double)F[3].x;
-                sm.Fy[4][PRP][lane] = (double)F[4].x;
+                sm.Fy[0][PRP][lane] = F[0].x;
+                sm.Fy[2][PRP][lane] = F[1].x;
+                sm.Fy[3][PRP][lane] = F[2].x;
+                sm.Fy[1][PRP][lane] = F[3].x;
+                sm.Fy[4][PRP][lane] = F[4].x;
                 if (lane < PTY) {
-                    double* const fxe = reinterpret_cast<double*>(&sm.Fx[0][lane >> 1][PTX]) + (lane & 1);
-                    constexpr int FXF2 = 2 * PRP * (PTX + 1);   // double stride of Fx per field
+                    float* const fxe = reinterpret_cast<float*>(&sm.Fx[0][lane >> 1][PTX]) + (lane & 1);
+                    constexpr int FXF2 = 2 * PRP * (PTX + 1);   // float stride of Fx per field
 #pragma unroll
-                    for (int f = 0; f < 5; f++) fxe[f * FXF2] = (double)F[f].y;
+                    for (int f = 0; f < 5; f++) fxe[f * FXF2] = F[f].y;
                 }
             }
             if (k + 1 < kend) {
