@@ -165,7 +165,8 @@ __device__ __forceinline__ int recover(double rho, double mx, double my, double 
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(ir) : "d"(rho));
     ir = __fma_rn(ir, __fma_rn(-rho, ir, 1.0), ir);
     double vx = __dmul_rn(mx, ir), vy = __dmul_rn(my, ir), vz = __dmul_rn(mz, ir);
-    const double m2 = __fma_rn(mz, vz, __fma_rn(my, vy, __dmul_rn(mx, vx)));
+    // (m.m)/rho with m.m formed first: it does not wait for the reciprocal, which shortens the dependent chain
+    const double m2 = __dmul_rn(__fma_rn(mz, mz, __fma_rn(my, my, __dmul_rn(mx, mx))), ir);
     double p = __dmul_rn(gm1, __fma_rn(-0.5, m2, e));
     const bool lo_p = p < KH_P_FLOOR;
     p = lo_p ? KH_P_FLOOR : p;

@@ -42,7 +42,7 @@ using pr::Gas;
 #define KH_CVT(x) ((double)(x))
 #endif
 #ifndef KH_TMA_UNROLL
-#define KH_TMA_UNROLL 2
+#define KH_TMA_UNROLL 4
 #endif
 constexpr int PTX = pr::PTX;       // 32
 #ifndef KH_TMA_PTY
@@ -62,10 +62,10 @@ constexpr int NTHREADS = NWARPS * 32;
 constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (register rotation becomes renaming)
 // register split of the three warpgroups (setmaxnreg): per scheduler 2 main warps + 1 auxiliary warp <= 16384
 #ifndef KH_TMA_MAIN_REGS
-#define KH_TMA_MAIN_REGS 184
+#define KH_TMA_MAIN_REGS 208
 #endif
 #ifndef KH_TMA_HALO_REGS
-#define KH_TMA_HALO_REGS 136
+#define KH_TMA_HALO_REGS 72
 #endif
 #define KH_TMA_STR2(x) #x
 #define KH_TMA_STR(x) KH_TMA_STR2(x)
