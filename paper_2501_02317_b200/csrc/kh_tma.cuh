@@ -72,7 +72,10 @@ constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (regist
 
 template <int STAGE>
 struct Cfg {
-    static constexpr int NSLOT = (STAGE == 1) ? 5 : 4;   // raw ring depth (stage 2 shares the space with U0)
+#ifndef KH_TMA_NSLOT2
+#define KH_TMA_NSLOT2 5
+#endif
+    static constexpr int NSLOT = (STAGE == 1) ? 5 : KH_TMA_NSLOT2;   // raw ring depth
     static constexpr int NU0 = (STAGE == 2) ? 2 : 0;
     static constexpr int NHALO = (STAGE == 2 && BLOCKS_PER_SM == 2) ? 2 : 3;   // halo ring depth
 };
@@ -835,10 +838,11 @@ inline void build_maps(StageMaps* sm, const double* A, const double* B, const Gr
 
 inline int auto_zchunk(const Grid& g)
 {
-    // >= ~12 waves of thread blocks over the 148 SMs, slabs of >= 32 planes
+    // >= ~6 waves of thread blocks over the 148 SMs (the tail of the last wave costs ~1 %), slabs of >= 32 planes
+    // (every slab converts two extra planes and primes its pipeline: ~3 planes of overhead)
     const long long tiles = (long long)(g.n[0] / PTX) * (g.n[1] / PTY);
     int chunk = g.n[2];
-    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * BLOCKS_PER_SM * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * BLOCKS_PER_SM * 6) chunk = (chunk + 1) / 2;
     return chunk;
 }
 
