@@ -53,15 +53,9 @@ __device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ f2 max0(f2 a) { return make_float2(fmaxf(a.x, 0.0f), fmaxf(a.y, 0.0f)); }
 __device__ __forceinline__ f2 maxs(f2 a, float s) { return make_float2(fmaxf(a.x, s), fmaxf(a.y, s)); }
-#ifdef KH_WHATIF_NOMUFU
-__device__ __forceinline__ f2 rcp2(f2 a) { return __ffma2_rn(a, make_float2(-1.f, -1.f), make_float2(2.f, 2.f)); }
-__device__ __forceinline__ f2 sqrt2(f2 a) { return __ffma2_rn(a, make_float2(.5f, .5f), make_float2(.5f, .5f)); }
-__device__ __forceinline__ f2 rsqrt2(f2 a) { return __ffma2_rn(a, make_float2(-.5f, -.5f), make_float2(1.5f, 1.5f)); }
-#else
 __device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(rcp_(a.x), rcp_(a.y)); }
 __device__ __forceinline__ f2 sqrt2(f2 a) { return make_float2(sqrt_(a.x), sqrt_(a.y)); }
 __device__ __forceinline__ f2 rsqrt2(f2 a) { return make_float2(rsqrt_(a.x), rsqrt_(a.y)); }
-#endif
 __device__ __forceinline__ f2 sel(bool cx, bool cy, f2 a, f2 b) { return make_float2(cx ? a.x : b.x, cy ? a.y : b.y); }
 __device__ __forceinline__ f2 mm2(f2 a, f2 b) { return make_float2(minmod(a.x, b.x), minmod(a.y, b.y)); }
 

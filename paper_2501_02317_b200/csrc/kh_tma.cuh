@@ -36,11 +36,6 @@ using pr::face_flux2;
 using pr::recover;
 using pr::Gas;
 
-#ifdef KH_WHATIF_NOF2F   // timing experiment only (wrong results): no fp32 -> fp64 conversion instructions
-#define KH_CVT(x) __hiloint2double(__float_as_int(x), 0)
-#else
-#define KH_CVT(x) ((double)(x))
-#endif
 #ifndef KH_TMA_UNROLL
 #define KH_TMA_UNROLL 4
 #endif
@@ -434,13 +429,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    Fzhi[f] = make_double2(__dmul_rn(dtdz, KH_CVT(F[f].x)), __dmul_rn(dtdz, KH_CVT(F[f].y)));
+                    Fzhi[f] = make_double2(__dmul_rn(dtdz, (double)F[f].x), __dmul_rn(dtdz, (double)F[f].y));
                     dU[f] = make_double2(__dadd_rn(Fzlo[f].x, -Fzhi[f].x), __dadd_rn(Fzlo[f].y, -Fzhi[f].y));
                 }
                 from_normal<0>(Fn[1], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double2 fd = make_double2(KH_CVT(F[f].x), KH_CVT(F[f].y));
+                    const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
                     fxs[f * QXF] = F[f];
                     dU[f].x = __fma_rn(dtdx, fd.x, dU[f].x);
                     dU[f].y = __fma_rn(dtdx, fd.y, dU[f].y);
@@ -448,7 +443,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<1>(Fn[2], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double flo = KH_CVT(F[f].x), fin = KH_CVT(F[f].y);
+                    const double flo = (double)F[f].x, fin = (double)F[f].y;
                     fys[f * QYF] = F[f].x;
                     dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin), dU[f].x);
                     dU[f].y = __fma_rn(dtdy, fin, dU[f].y);
