@@ -18,7 +18,7 @@
 // Phases per plane k (as in kh_pair.cuh):
 //                                                                            | barrier 1
 //      [producer: store plane k-1, then refill its slot with plane k-1+NSLOT; halo plane k+3; U0(k+1)]
-//   B) z/x/y fluxes of plane k, conversion of plane k+2, tile of plane k+1   | barrier 2
+//   B) z/x/y fluxes of plane k, conversion of plane k+3, tile of plane k+1   | barrier 2
 //   C) fp64 update of plane k, written in place; Heun average and CFL rate (stage 2)
 //   A) of plane k+1, fused with C: x/y slopes from the primitive tile, left states published
 #pragma once
@@ -67,10 +67,9 @@ constexpr int UNROLL = KH_TMA_UNROLL;  // planes per trip of the z march (regist
 
 template <int STAGE>
 struct Cfg {
-#ifndef KH_TMA_NSLOT2
-#define KH_TMA_NSLOT2 5
-#endif
-    static constexpr int NSLOT = (STAGE == 1) ? 5 : KH_TMA_NSLOT2;   // raw ring depth
+    // raw ring depth: planes k (updated in place, then stored), k+1, k+2 (held for their update), k+3 (being converted)
+    // and one being refilled
+    static constexpr int NSLOT = 5;
     static constexpr int NU0 = (STAGE == 2) ? 2 : 0;
     static constexpr int NHALO = (STAGE == 2 && BLOCKS_PER_SM == 2) ? 2 : 3;   // halo ring depth
 };
@@ -369,14 +368,15 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
         };
 
-        // ---- prologue: planes kbeg-2, kbeg-1, kbeg (ring slots 0, 1, 2, first fill: parity 0) ----
-        f2 Wa[5], Wb[5], QLz[5];   // W(k), W(k+1), left state of z face k+1/2
+        // ---- prologue: planes kbeg-2 .. kbeg+1 (ring slots 0 .. 3, first fill: parity 0) ----
+        f2 Wa[5], Wb[5], Wn[5], QLz[5];   // W(k), W(k+1), W(k+2), left state of z face k+1/2
         double2 Fzlo[5];           // dt/dz * flux through z face k-1/2
         {
             f2 Wm[5];
             convert(kbeg - 2, 0, 0u, Wm, false);
             convert(kbeg - 1, 1, 0u, Wa, false);
             convert(kbeg, 2, 0u, Wb, true);
+            convert(kbeg + 1, 3, 0u, Wn, kbeg + 1 < kend);
 #pragma unroll
             for (int f = 0; f < 5; f++) {
                 f2 qR;
@@ -384,9 +384,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 Fzlo[f] = make_double2(0.0, 0.0);
             }
         }
-        // ring positions of the planes k+2 (converted) and k (updated) at the first iteration k = kfirst
-        int s_conv = 3 % NSLOT, s_upd = 1;
-        unsigned par_conv = (3 >= NSLOT) ? 1u : 0u;
+        // ring positions of the planes k+3 (converted) and k (updated) at the first iteration k = kfirst
+        constexpr int QCONV = 4;   // ring index of the plane converted in the first iteration (kbeg+2)
+        int s_conv = QCONV % NSLOT, s_upd = 1;
+        unsigned par_conv = (QCONV >= NSLOT) ? 1u : 0u;
 
         f2 QRx[5], QRy[5];
         float QLyo[5];  // left state of the face between the pair's two cells
@@ -402,10 +403,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             // The z, x and y Riemann problems of the pair are independent: they are solved in lock step
             // (hllc2n).  In the priming iteration the x / y inputs are not valid yet; those results are
             // computed all the same (one basic block) and never used.
-            f2 Wn[5];
             double2 Fzhi[5];
+            f2 Wn2[5];
             {
-                convert(k + 2, s_conv, par_conv, Wn, k + 2 < kend);
                 f2 L[3][5], R[3][5], Fn[3][5], F[5];
                 {
                     f2 qL[5], qR[5];
@@ -426,6 +426,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     to_normal<1>(QRy, R[2]);
                 }
                 hllc2n<3>(L, R, gas, Fn);
+                // plane k+3 (Sec. 3.1): converted here, where the registers of the Riemann solver are free again; its
+                // fp64 chain overlaps the flux accumulation below and phase B(k+1) starts with W(k+3) at hand
+                convert(k + 3, s_conv, par_conv, Wn2, k + 3 < kend);
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
@@ -539,7 +542,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             }
             // rotate the z march and the ring
 #pragma unroll
-            for (int f = 0; f < 5; f++) { Wa[f] = Wb[f]; Wb[f] = Wn[f]; Fzlo[f] = Fzhi[f]; }
+            for (int f = 0; f < 5; f++) {
+                Wa[f] = Wb[f]; Wb[f] = Wn[f]; Fzlo[f] = Fzhi[f];
+                Wn[f] = Wn2[f];
+            }
             if (++s_conv == NSLOT) { s_conv = 0; par_conv ^= 1u; }
             if (++s_upd == NSLOT) s_upd = 0;
         }
@@ -695,7 +701,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         const HaloSide yhi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
         const HaloSide xlo = halo_side(i0 - 2, nx, g.bc[0], g.bc[1]);
         const HaloSide xhi = halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
-        const int plast = kend + 1;  // last plane the z stencil of this slab needs
+        const int plast = kend + 2;  // planes up to kend+1 feed the z stencil; the main warps convert one plane further
+                                     // (unconditionally: straight-line code), so that one is loaded too
         auto load_raw = [&](int p, int slot) {
             int rz;
             const int sk = bc_source(p, nz, g.bc[4], g.bc[5], rz);
