@@ -462,6 +462,18 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) wt[f * WTF] = Wb[f];
             }
+            // The thread's own fp64 data for the update (nobody else touches these entries) are fetched BEFORE the barrier:
+            // their latency hides behind the barrier wait and they stay out of the load burst that follows it.
+            double* const su = raw0 + s_upd * RAWS;
+            const double* const s0 = u00 + ((k - kbeg) & 1) * RAWS;
+            if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
+            double ua[5], ub[5], va[5], vb[5];
+#pragma unroll
+            for (int f = 0; f < 5; f++) {
+                ua[f] = su[f * RAWF];
+                ub[f] = su[f * RAWF + PTX];
+                if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
+            }
             KH_PROBE(3)
             block_bar();
             // ---------------- phase C of plane k + phase A of plane k+1, as one block of straight-line code ----------
@@ -473,21 +485,14 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             // data and in the last iteration A does: both results are never used (the in-place write then lands in
             // a slot whose plane has been converted already and is refilled later).
             {
-                double* su = raw0 + s_upd * RAWS;
-                const double* s0 = u00 + ((k - kbeg) & 1) * RAWS;
-                if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
                 f2 fxh[5];
                 float fyh[5];
-                double ua[5], ub[5], va[5], vb[5];
                 f2 xm[5], xp[5], qLx[5], qLy[5];
                 float below[5], above[5];   // rows 2w-1 and 2w+2: the near halves of the neighbouring row pairs
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     fxh[f] = fxs[f * QXF + 1];
                     fyh[f] = fys[f * QYF + PTX];
-                    ua[f] = su[f * RAWF];
-                    ub[f] = su[f * RAWF + PTX];
-                    if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
                 }
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
