@@ -47,6 +47,8 @@ def workload(name: str):
         return inputs.point_blast_3d(256, nsteps=50), "C4 3D point blast 256^3 outflow gamma=5/3"
     if name == "C3":
         return inputs.shear_layer_2d(2048, seed=3, nsteps=100), "C3 2D shear layer 2048^2 periodic gamma=5/3"
+    if name == "implosion":
+        return inputs.implosion_2d(2048, nsteps=100), "Liska-Wendroff implosion 2048^2, reflecting walls, gamma=1.4 (PAPER Sec. 4.4)"
     raise SystemExit(f"unknown workload {name}")
 
 

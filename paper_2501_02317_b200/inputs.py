@@ -231,6 +231,23 @@ def turbulence_3d(n: int = 512, seed: int = 5, nsteps: int = 20, gamma: float = 
                    nsteps=nsteps, meta=dict(n=n, seed=seed))
 
 
+# ----------------------------------------------------------------------------- Liska-Wendroff implosion
+def implosion_2d(n: int = 400, nsteps: int = 0, t_end: float = 0.045 / 0.3) -> Problem:
+    """Sec. 4.4, Eq. 7: gamma = 1.4, (rho, p) = (0.125, 0.14) where x + y < 0.15 and (1, 1)
+    elsewhere, gas at rest, reflecting walls on all four sides.  The test lives on the box [0, 0.3]^2; the Euler
+    equations carry no length scale, so it is set up here on the unit box used everywhere in this package
+    (corner region x + y < 1/2) and times scale by 1/0.3 (t = 0.045 there is t = 0.15 here).  Cell centres
+    exactly on the diagonal x + y = 1/2 do not occur for even n."""
+    gamma = 1.4
+    x = centres(n)
+    corner = (x[None, :] + x[:, None]) < 0.5          # [y, x]
+    rho = np.where(corner, 0.125, 1.0)[None]
+    p = np.where(corner, 0.14, 1.0)[None]
+    U = prim_to_cons(rho, p, 0.0, 0.0, 0.0, gamma)
+    return Problem("implosion_2d", np.ascontiguousarray(U), gamma, (REFLECT, REFLECT, REFLECT, REFLECT, PERIODIC, PERIODIC),
+                   nsteps=nsteps, t_end=(0.0 if nsteps else t_end), meta=dict(n=n))
+
+
 # ----------------------------------------------------------------------------- misc small cases
 def random_smooth(nx: int, ny: int, nz: int, seed: int, gamma: float = 1.4, bc=(PERIODIC,) * 6,
                   amp: float = 0.3) -> Problem:

@@ -422,3 +422,52 @@ def test_c5_full_size_sampled_against_oracle():
         got = Ug[:, kc][:, :, jc][:, :, :, ic]
         err = rel_l1_fields(got, ref)
         assert max(err) <= TOL[MIXED], ((k0, j0, i0), err)
+
+
+# --------------------------------------------------------------------------- Sec. 4.4 Liska-Wendroff implosion (reflecting walls)
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_implosion_2d_reduced(prec):
+    """Eq. 7 at 128^2 in a box of reflecting walls (BC code 3 on all four sides): parity with the
+    oracle while the flow is still deterministic, closed-box conservation of mass and energy, and in all-fp64 mode
+    the diagonal symmetry rho(x,y) = rho(y,x), m_x(x,y) = m_y(y,x) to rounding."""
+    n, nsteps = 128, 80
+    pr = inputs.implosion_2d(n, nsteps=nsteps)
+    Uo = pr.U.copy()
+    _, _, hits_o = oracle.run(Uo, pr.gamma, pr.bc, 0.4, nsteps)
+    h = make(pr, prec)
+    T0 = h.totals()
+    h.run(0.4, nsteps)
+    T1 = h.totals()
+    Ug = h.get_state()
+    hits = h.floor_hits()
+    h.destroy()
+    assert hits == 0 and hits_o == 0
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+    assert abs(T1[0] - T0[0]) <= 1e-13 * T0[0] and abs(T1[4] - T0[4]) <= 1e-13 * T0[4]
+    if prec == FP64:
+        rho, mx, my, e = Ug[0][0], Ug[1][0], Ug[2][0], Ug[4][0]
+        assert np.abs(rho - rho.T).max() <= 1e-12
+        assert np.abs(mx - my.T).max() <= 1e-12
+        assert np.abs(e - e.T).max() <= 1e-12
+
+
+def test_implosion_extruded_through_the_tma_kernel():
+    """The same problem extruded along z (periodic): the 3D TMA kernel with reflecting boxes in x and y must reproduce
+    the 2D oracle run in every z plane, with the z momentum exactly zero."""
+    n, nzz, nsteps = 64, 8, 40
+    pr2 = inputs.implosion_2d(n, nsteps=nsteps)
+    Uo = pr2.U.copy()
+    U3 = np.ascontiguousarray(np.repeat(pr2.U, nzz, axis=1))
+    pr3 = inputs.Problem("implosion_extruded", U3, pr2.gamma, pr2.bc)
+    h = make(pr3, MIXED, TMA)
+    h.set_spacing(1.0 / n, 1.0 / n, 1.0 / n)
+    for _ in range(nsteps):
+        dt = oracle.cfl_dt(Uo, pr2.gamma, 0.4)
+        oracle.step(Uo, pr2.gamma, pr2.bc, dt)
+        h.step(dt)
+    Ug = h.get_state()
+    h.destroy()
+    assert np.all(Ug[3] == 0.0)
+    for k in range(nzz):
+        assert np.array_equal(Ug[:, k], Ug[:, 0])          # every plane the same bits
+    assert max(rel_l1_fields(Ug[:, :1], Uo)) <= TOL[MIXED]
