@@ -57,6 +57,10 @@ def lib() -> ctypes.CDLL:
         L.orc_flux_divergence.argtypes = [dp, i, i, i, d, ip, d, d, d, dp, llp]
         L.orc_step.restype = i
         L.orc_step.argtypes = [dp, i, i, i, d, ip, d, d, d, d, llp]
+        L.orc_step_vl.restype = i
+        L.orc_step_vl.argtypes = [dp, i, i, i, d, ip, d, d, d, d, llp]
+        L.orc_run_vl.restype = i
+        L.orc_run_vl.argtypes = [dp, i, i, i, d, ip, d, d, d, d, i, d, dp, llp]
         L.orc_cfl_dt.restype = d
         L.orc_cfl_dt.argtypes = [dp, i, i, i, d, d, d, d, d, llp]
         L.orc_run.restype = i
@@ -128,12 +132,17 @@ def flux_divergence(U: np.ndarray, gamma, bc, spacing=None):
     return L, hits.value
 
 
-def step(U: np.ndarray, gamma, bc, dt, spacing=None) -> int:
-    """One Heun step in place; returns the number of floor activations."""
+HEUN, VANLEER = "heun", "vanleer"   # Sec. 3.3
+
+
+def step(U: np.ndarray, gamma, bc, dt, spacing=None, integrator=HEUN) -> int:
+    """One step in place (Heun by default, van Leer predictor-corrector on request); returns the number of floor
+    activations."""
     nx, ny, nz = _chk(U)
     dx, dy, dz = spacing or default_spacing(nx, ny, nz)
     hits = ctypes.c_longlong(0)
-    rc = lib().orc_step(_dp(U), nx, ny, nz, gamma, _bc(bc), dx, dy, dz, dt, ctypes.byref(hits))
+    fn = lib().orc_step_vl if integrator == VANLEER else lib().orc_step
+    rc = fn(_dp(U), nx, ny, nz, gamma, _bc(bc), dx, dy, dz, dt, ctypes.byref(hits))
     if rc:
         raise MemoryError("oracle allocation failed")
     return hits.value
@@ -146,13 +155,14 @@ def cfl_dt(U: np.ndarray, gamma, cfl, spacing=None) -> float:
     return lib().orc_cfl_dt(_dp(U), nx, ny, nz, gamma, dx, dy, dz, cfl, ctypes.byref(hits))
 
 
-def run(U: np.ndarray, gamma, bc, cfl, nsteps, t0=0.0, t_end=0.0, spacing=None):
+def run(U: np.ndarray, gamma, bc, cfl, nsteps, t0=0.0, t_end=0.0, spacing=None, integrator=HEUN):
     """Advance in place; returns (t, steps_taken, floor_hits)."""
     nx, ny, nz = _chk(U)
     dx, dy, dz = spacing or default_spacing(nx, ny, nz)
     t = ctypes.c_double(t0)
     hits = ctypes.c_longlong(0)
-    n = lib().orc_run(_dp(U), nx, ny, nz, gamma, _bc(bc), dx, dy, dz, cfl, nsteps, t_end,
+    fn = lib().orc_run_vl if integrator == VANLEER else lib().orc_run
+    n = fn(_dp(U), nx, ny, nz, gamma, _bc(bc), dx, dy, dz, cfl, nsteps, t_end,
                       ctypes.byref(t), ctypes.byref(hits))
     if n < 0:
         raise MemoryError("oracle allocation failed")

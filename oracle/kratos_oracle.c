@@ -20,8 +20,9 @@
  * with the paper's N^-2 order, exact conservation, uniform-state fixed point,
  * stationary/moving contact, consistency, axis interchange / mirror, monotonicity,
  * independent brute force).  Parity UNPINNED for: Kratos' own (unpublished) choice of
- * CFL formula (S1), of the p* estimate entering Eq. 5 (S3) and of floors (S6) -- no
- * output of the real code exists to compare against.
+ * CFL formula (S1), of the p* estimate entering Eq. 5 (S3), of floors (S6) and of the
+ * van Leer integrator's sub-steps (S15, orc_step_vl) -- no output of the real code exists
+ * to compare against.
  *
  * No blocking, fusion or reordering beyond what the paper's algorithm states; the
  * only concession to speed is "#pragma omp parallel for" on outermost loops, which
@@ -213,8 +214,10 @@ void orc_fill_ghosts_axis(double *W, int nx, int ny, int nz, int d, int bc_lo, i
  *   3. per active axis: PLM with minmod slopes, Delta x in the denominator
  *      (Eq. 3), then HLLC at every face.
  * Lout has the layout of U.  Returns 0, or -2 if allocation fails. */
-int orc_flux_divergence(const double *U, int nx, int ny, int nz, double gamma, const int bc[6],
-                        double dx, double dy, double dz, double *Lout, long long *floor_hits)
+/* order = 2: slope-limited PLM (Eq. 3); order = 1: piecewise-constant states (all slopes 0), used by the
+ * predictor of the van Leer integrator (reading S15). */
+static int flux_divergence_order(const double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+                                 double dx, double dy, double dz, double *Lout, long long *floor_hits, int order)
 {
     orc_geom G = make_geom(nx, ny, nz);
     const long long N = (long long)nx * ny * nz;
@@ -273,7 +276,7 @@ int orc_flux_divergence(const double *U, int nx, int ny, int nz, double gamma, c
                     for (int m = 0; m < 5; m++) {
                         const double qm = q[5 * (i - 1 + NGH) + m], q0 = q[5 * (i + NGH) + m],
                                      qp = q[5 * (i + 1 + NGH) + m];
-                        sig[5 * (i + NGH) + m] = orc_minmod((q0 - qm) / h[d], (qp - q0) / h[d]);
+                        sig[5 * (i + NGH) + m] = (order == 1) ? 0.0 : orc_minmod((q0 - qm) / h[d], (qp - q0) / h[d]);
                     }
                 /* faces i+1/2, i = -1..n-1 */
                 for (int i = -1; i <= n - 1; i++) {
@@ -308,6 +311,38 @@ int orc_flux_divergence(const double *U, int nx, int ny, int nz, double gamma, c
 /* Sec. 3.3: one Heun (RK2) step of length dt.
  *   U1 = U0 + dt L(U0);  U = 1/2 U0 + 1/2 (U1 + dt L(U1))     (predictor enters with weight 1/2)
  * U is updated in place. */
+int orc_flux_divergence(const double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+                        double dx, double dy, double dz, double *Lout, long long *floor_hits)
+{
+    return flux_divergence_order(U, nx, ny, nz, gamma, bc, dx, dy, dz, Lout, floor_hits, 2);
+}
+
+/* Sec. 3.3: the "memory-optimized second order van Leer integrator", whose prediction
+ * sub-step does not enter the final result directly.  The paper prints no formulas; reading S15:
+ * the predictor-corrector of van Leer as used in finite-volume codes,
+ *     U^{n+1/2} = U^n + (dt/2) L_1(U^n)        L_1: piecewise-constant states at the faces (first order)
+ *     U^{n+1}   = U^n +  dt    L_2(U^{n+1/2})  L_2: slope-limited PLM + HLLC, as in the Heun stages
+ * Same ghost rules, floors and CFL formula as the Heun path.  Conservative: U^n only ever receives flux
+ * differences.  Parity with Kratos' own choice is UNPINNED. */
+int orc_step_vl(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+                double dx, double dy, double dz, double dt, long long *floor_hits)
+{
+    const long long N5 = 5LL * nx * ny * nz;
+    double *L = (double *)malloc(sizeof(double) * N5);
+    double *Uh = (double *)malloc(sizeof(double) * N5);
+    if (!L || !Uh) { free(L); free(Uh); return -2; }
+    int rc = flux_divergence_order(U, nx, ny, nz, gamma, bc, dx, dy, dz, L, floor_hits, 1);
+    if (rc) { free(L); free(Uh); return rc; }
+#pragma omp parallel for
+    for (long long c = 0; c < N5; c++) Uh[c] = U[c] + 0.5 * dt * L[c];
+    rc = flux_divergence_order(Uh, nx, ny, nz, gamma, bc, dx, dy, dz, L, floor_hits, 2);
+    if (rc) { free(L); free(Uh); return rc; }
+#pragma omp parallel for
+    for (long long c = 0; c < N5; c++) U[c] = U[c] + dt * L[c];
+    free(L); free(Uh);
+    return 0;
+}
+
 int orc_step(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
              double dx, double dy, double dz, double dt, long long *floor_hits)
 {
@@ -357,9 +392,9 @@ double orc_cfl_dt(const double *U, int nx, int ny, int nz, double gamma,
 /* ------------------------------------------------------------------------- */
 /* Driver: repeat { dt = cfl_dt; clip to t_end; step } for at most nsteps steps or
  * until t reaches t_end (t_end <= 0: no end time).  Returns steps taken, <0 on error. */
-int orc_run(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
-            double dx, double dy, double dz, double cfl, int nsteps, double t_end,
-            double *t_inout, long long *floor_hits)
+static int run_with(int integrator, double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+                    double dx, double dy, double dz, double cfl, int nsteps, double t_end,
+                    double *t_inout, long long *floor_hits)
 {
     double t = *t_inout;
     int s = 0;
@@ -367,12 +402,27 @@ int orc_run(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
         if (t_end > 0.0 && t >= t_end) break;
         double dt = orc_cfl_dt(U, nx, ny, nz, gamma, dx, dy, dz, cfl, floor_hits);
         if (t_end > 0.0 && t + dt > t_end) dt = t_end - t;
-        int rc = orc_step(U, nx, ny, nz, gamma, bc, dx, dy, dz, dt, floor_hits);
+        int rc = integrator ? orc_step_vl(U, nx, ny, nz, gamma, bc, dx, dy, dz, dt, floor_hits)
+                            : orc_step(U, nx, ny, nz, gamma, bc, dx, dy, dz, dt, floor_hits);
         if (rc) return rc;
         t += dt;
     }
     *t_inout = t;
     return s;
+}
+
+int orc_run(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+            double dx, double dy, double dz, double cfl, int nsteps, double t_end,
+            double *t_inout, long long *floor_hits)
+{
+    return run_with(0, U, nx, ny, nz, gamma, bc, dx, dy, dz, cfl, nsteps, t_end, t_inout, floor_hits);
+}
+
+int orc_run_vl(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
+               double dx, double dy, double dz, double cfl, int nsteps, double t_end,
+               double *t_inout, long long *floor_hits)
+{
+    return run_with(1, U, nx, ny, nz, gamma, bc, dx, dy, dz, cfl, nsteps, t_end, t_inout, floor_hits);
 }
 
 /* ------------------------------------------------------------------------- */

@@ -585,3 +585,98 @@ def test_implosion_diagonal_symmetry_and_closed_box_conservation():
         oracle.step(U1, pr.gamma, pr.bc, dt)
         oracle.step(big, pr.gamma, pr.bc, dt, spacing=(1.0 / n, 1.0 / n, 1.0))
     assert np.abs(big[:, :, n:, :] - U1).max() <= 1e-13
+
+
+# --------------------------------------------------------------------------- Sec. 3.3 van Leer integrator (reading S15)
+VL = oracle.VANLEER
+
+
+def test_vanleer_local_error_scales_as_dt2_dx():
+    """"second order van Leer integrator".  Its predictor is first order in space (reading S15), so
+    against a finely sub-stepped integration of the PLM operator the ONE-step error is O(dt^2 dx) + O(dt^3): it falls
+    ~4x when dt is halved and ~2x when dx is halved at fixed dt -- i.e. second order when dt and dx shrink together
+    (the wave tests below).  A wrong half-step weight leaves an O(dt^2) error that does not shrink with dx."""
+    bc = (P,) * 6
+
+    def state(n):
+        x = inputs.centres(n)
+        return inputs.prim_to_cons((1 + 0.2 * np.sin(2 * np.pi * x)).reshape(1, 1, -1),
+                                   (1 + 0.1 * np.cos(2 * np.pi * x)).reshape(1, 1, -1),
+                                   (0.3 * np.sin(2 * np.pi * x + 1)).reshape(1, 1, -1), 0.0, 0.0, 1.4)
+
+    def err(n, T):
+        ref = state(n)
+        for _ in range(64):
+            oracle.step(ref, 1.4, bc, T / 64)
+        U = state(n)
+        oracle.step(U, 1.4, bc, T, integrator=VL)
+        return np.abs(U - ref).mean()
+
+    dt = 2e-3
+    e_a, e_b, e_c = err(64, dt), err(64, dt / 2), err(128, dt)
+    assert 3.2 < e_a / e_b < 4.8, (e_a, e_b)
+    assert 1.6 < e_a / e_c < 2.6, (e_a, e_c)
+
+
+@pytest.mark.parametrize("kind", ["contact", "shear"])
+def test_vanleer_wave_convergence_order(kind):
+    """Same closed-form test as P2: second order in space and time."""
+    errs = []
+    ns = (64, 128, 256)
+    for n in ns:
+        pr = inputs.wave_1d(n, kind)
+        U = pr.U.copy()
+        t, _, hits = oracle.run(U, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 1.0, integrator=VL)
+        assert t == pytest.approx(1.0, abs=1e-14) and hits == 0
+        if kind == "contact":
+            errs.append(paper_l1(U[0], pr.U[0]))
+        else:
+            errs.append(paper_l1(U[2] / U[0], pr.U[2] / pr.U[0]))
+    orders = [math.log2(errs[i] / errs[i + 1]) for i in range(len(ns) - 1)]
+    assert all(1.6 < o < 2.3 for o in orders), (errs, orders)
+
+
+def test_vanleer_exact_riemann_convergence_conservation_and_fixed_point():
+    # P1: converges to the exact Riemann solution
+    errs = []
+    for n in (128, 256, 512):
+        pr = inputs.riemann_1d(1, n)
+        U = pr.U.copy()
+        oracle.run(U, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.2, integrator=VL)
+        (rl, ul, pl), (rr, ur, prr) = pr.meta["left"], pr.meta["right"]
+        xi = (inputs.centres(n) - 0.5) / 0.2
+        rho_e, _, _ = er.sample(xi, rl, ul, pl, rr, ur, prr, pr.gamma)
+        errs.append(np.abs(U[0, 0, 0] - rho_e).mean())
+    assert all(0.55 < math.log2(errs[i] / errs[i + 1]) < 1.1 for i in range(2)), errs
+    # P3: "keeping the conservation law up to the full machine accuracy" (PAPER.md:274)
+    pr = inputs.random_smooth(20, 12, 9, seed=4)
+    U = pr.U.copy()
+    T0 = oracle.totals(U)
+    A0 = np.array([np.abs(U[m]).sum() for m in range(5)])
+    oracle.run(U, pr.gamma, pr.bc, 0.4, 25, integrator=VL)
+    T1 = oracle.totals(U)
+    assert (np.abs(T1 - T0) / np.maximum(np.abs(T0), A0)).max() <= 1e-13
+    # P4: a uniform state is a bitwise fixed point
+    U0 = inputs.prim_to_cons(np.full((6, 8, 10), 1.3), 0.7, 0.4, -1.1, 2.2, 1.4)
+    for bc in ((P,) * 6, (F,) * 6, (R,) * 6):
+        Uu = np.ascontiguousarray(U0.copy())
+        if bc[0] == R:
+            Uu = np.ascontiguousarray(inputs.prim_to_cons(np.full((6, 8, 10), 1.3), 0.7, 0.0, 0.0, 0.0, 1.4))
+        ref = Uu.copy()
+        for _ in range(3):
+            oracle.step(Uu, 1.4, bc, 1e-3, integrator=VL)
+        assert np.array_equal(Uu, ref)
+
+
+def test_vanleer_and_heun_agree_to_second_order():
+    """Two second-order integrators of the same equations: their difference after a fixed time shrinks at least like
+    dt^2 ~ N^-2 on a smooth problem (a wrong half-step weight leaves a first-order difference)."""
+    diffs = []
+    for n in (32, 64, 128):
+        pr = inputs.advected_wave_2d(n, t_end=0.25)
+        a, b = pr.U.copy(), pr.U.copy()
+        oracle.run(a, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.25)
+        oracle.run(b, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.25, integrator=VL)
+        diffs.append(np.abs(a[0] - b[0]).mean())
+    orders = [math.log2(diffs[i] / diffs[i + 1]) for i in range(2)]
+    assert all(o > 1.4 for o in orders), (diffs, orders)   # minmod clips the extrema: the L1 order approaches 2 from below
