@@ -57,6 +57,9 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
 #define KRATOS_PREC_MIXED 0 /* float_t = fp32 (reconstruction, Riemann), float2_t = fp64 (state, update) */
 #define KRATOS_PREC_FP64 1  /* float_t = float2_t = fp64 */
 #define KRATOS_INTEGRATOR_HEUN (0 << 4)
+#define KRATOS_INTEGRATOR_VANLEER (1 << 4) /* predictor-corrector of Sec. 3.3: predictor kept as float_t
+                                             primitives (20 B per cell in mixed precision instead of a second fp64 state);
+                                             served by the general one-thread-per-cell kernels */
 
 /* boundary codes, the paper's list order */
 #define KRATOS_BC_PERIODIC 0 /* communication boundary onto the same block: wrap copy */

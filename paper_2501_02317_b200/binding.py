@@ -18,6 +18,7 @@ from . import build as _build
 
 PREC_MIXED, PREC_FP64 = 0, 1
 BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
+INTEGRATOR_HEUN, INTEGRATOR_VANLEER = 0 << 4, 1 << 4   # scheme word bits 4-5
 KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_ROLES, KERNEL_TMA = 0, 1, 2, 3, 4, 5
 OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
 
@@ -127,13 +128,13 @@ class KratosHydro:
     """One uniform block on the current CUDA device.  Method names mirror the C entry points."""
 
     def __init__(self, nx, ny, nz, gamma, bc, precision=PREC_MIXED, spacing=None, kernel=KERNEL_AUTO,
-                 stream=None):
+                 stream=None, integrator=INTEGRATOR_HEUN):
         L = load()
         self._L = L
         self.shape = (int(nx), int(ny), int(nz))
         self.ncell = int(nx) * int(ny) * int(nz)
         bc_arr = (ctypes.c_int * 6)(*[int(b) for b in bc])
-        self._h = L.kratos_hydro_create(int(nx), int(ny), int(nz), float(gamma), int(precision), bc_arr)
+        self._h = L.kratos_hydro_create(int(nx), int(ny), int(nz), float(gamma), int(precision) | int(integrator), bc_arr)
         if not self._h:
             raise KratosError(ERR_ARG, last_error())
         if spacing is not None:

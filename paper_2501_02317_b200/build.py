@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkratos_hydro.so")
 SOURCES = ["kh_api.cu"]
-HEADERS = ["kh_device.cuh", "kh_simple.cuh", "kh_tiled.cuh", "kh_pair.cuh", "kh_role.cuh", "kh_tma.cuh", "kh_reduce.cuh",
+HEADERS = ["kh_device.cuh", "kh_simple.cuh", "kh_tiled.cuh", "kh_pair.cuh", "kh_role.cuh", "kh_tma.cuh", "kh_vanleer.cuh", "kh_reduce.cuh",
            os.path.join("..", "..", "include", "kratos_hydro.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -16,6 +16,7 @@
 #include "kh_pair.cuh"
 #include "kh_role.cuh"
 #include "kh_tma.cuh"
+#include "kh_vanleer.cuh"
 
 using namespace kh;
 
@@ -44,12 +45,13 @@ enum { CFL_MAX_BLOCKS = 148 * 8 };
 struct kratos_hydro {
     Grid g;
     int prec;        // KRATOS_PREC_*
+    int integ;       // 0: Heun, 1: van Leer predictor-corrector
     int variant;     // resolved KRATOS_KERNEL_SIMPLE / _TILED
     bool tiled_ok;   // tiled kernel supports this block
     int zchunk;      // 0 = auto
     tma::StageMaps* maps;  // tensor maps of the TMA kernel (host; NULL when the block is not supported)
     double* U0;      // current state (device)
-    double* U1;      // predictor (device)
+    double* U1;      // Heun: predictor state, 5 N fp64.  van Leer: W^{n+1/2}, 5 N float_t primitives (device)
     Ctrl* ctrl;      // device
     Ctrl* h_ctrl;    // pinned host mirror
     dd* partial;     // totals scratch (device)
@@ -162,6 +164,16 @@ int launch_stage(kratos_hydro* h, int stage)
 int launch_both_stages(kratos_hydro* h)
 {
     int rc;
+    if (h->integ == 1) {  // van Leer: predictor into the float_t primitive array, corrector in place
+        for (int which = 1; which <= 2; which++) {
+            LaunchTimer lt(h, which == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
+            if (h->prec == KRATOS_PREC_MIXED) vl::launch_step<float>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
+            else                              vl::launch_step<double>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "van Leer sub-step %d launch: %s", which, cudaGetErrorString(e));
+        }
+        return KRATOS_OK;
+    }
     if (h->prec == KRATOS_PREC_MIXED) {
         if ((rc = launch_stage<float>(h, 1))) return rc;
         return launch_stage<float>(h, 2);
@@ -216,7 +228,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     if (!bc) { fail(KRATOS_ERR_ARG, "bc is NULL"); return nullptr; }
     if (!(gamma > 1.0) || !std::isfinite(gamma)) { fail(KRATOS_ERR_ARG, "gamma must be > 1"); return nullptr; }
     const int prec = scheme & 3, integ = (scheme >> 4) & 3;
-    if ((prec != KRATOS_PREC_MIXED && prec != KRATOS_PREC_FP64) || integ != 0 || (scheme & ~0x33)) {
+    if ((prec != KRATOS_PREC_MIXED && prec != KRATOS_PREC_FP64) || integ > 1 || (scheme & ~0x33)) {
         fail(KRATOS_ERR_ARG, "unsupported scheme word 0x%x", scheme);
         return nullptr;
     }
@@ -261,7 +273,8 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     }
     g.gamma = gamma;
     h->prec = prec;
-    h->tiled_ok = g.active[0] && g.active[1];
+    h->integ = integ;
+    h->tiled_ok = g.active[0] && g.active[1] && integ == 0;   // the fused stage kernels are the Heun path
     h->maps = nullptr;
     h->variant = auto_variant(h);
     h->zchunk = 0;
@@ -275,15 +288,18 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->ctrl = nullptr; h->h_ctrl = nullptr; h->partial = nullptr; h->d_tot = nullptr; h->p_partial = nullptr;
     h->tot_blocks = (int)((g.N + 255) / 256 < 592 ? (g.N + 255) / 256 : 592);
     const size_t bytes = sizeof(double) * 5 * (size_t)g.N;
+    // second array: the fp64 predictor of Heun, or the float_t primitives W^{n+1/2} of van Leer (PAPER.md:272:
+    // "saves up to ~1/3 of the device memory": 40 + 20 instead of 40 + 40 bytes per cell in mixed precision)
+    const size_t bytes1 = (integ == 1) ? (prec == KRATOS_PREC_MIXED ? sizeof(float) : sizeof(double)) * 5 * (size_t)g.N : bytes;
     cudaError_t e;
-    if ((e = cudaMalloc(&h->U0, bytes)) != cudaSuccess || (e = cudaMalloc(&h->U1, bytes)) != cudaSuccess ||
+    if ((e = cudaMalloc(&h->U0, bytes)) != cudaSuccess || (e = cudaMalloc(&h->U1, bytes1)) != cudaSuccess ||
         (e = cudaMalloc(&h->ctrl, sizeof(Ctrl))) != cudaSuccess ||
         (e = cudaMalloc(&h->partial, sizeof(dd) * 5 * h->tot_blocks)) != cudaSuccess ||
         (e = cudaMalloc(&h->d_tot, sizeof(double) * 5)) != cudaSuccess ||
         (e = cudaMalloc(&h->p_partial, sizeof(double) * CFL_MAX_BLOCKS)) != cudaSuccess ||
         (e = cudaMallocHost(&h->h_ctrl, sizeof(Ctrl) + 64)) != cudaSuccess ||
         (e = cudaMemset(h->ctrl, 0, sizeof(Ctrl))) != cudaSuccess ||
-        (e = cudaMemset(h->U0, 0, bytes)) != cudaSuccess || (e = cudaMemset(h->U1, 0, bytes)) != cudaSuccess) {
+        (e = cudaMemset(h->U0, 0, bytes)) != cudaSuccess || (e = cudaMemset(h->U1, 0, bytes1)) != cudaSuccess) {
         fail(e == cudaErrorMemoryAllocation ? KRATOS_ERR_ALLOC : KRATOS_ERR_CUDA, "create: %s", cudaGetErrorString(e));
         cudaGetLastError();
         kratos_hydro_destroy(h);
@@ -293,7 +309,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     pr::configure();
     rl::configure();
     tma::configure();
-    if (prec == KRATOS_PREC_MIXED && tma::supported(g)) {
+    if (prec == KRATOS_PREC_MIXED && integ == 0 && tma::supported(g)) {
         h->maps = new (std::nothrow) tma::StageMaps;
         if (h->maps) tma::build_maps(h->maps, h->U0, h->U1, g);
     }

@@ -471,3 +471,68 @@ def test_implosion_extruded_through_the_tma_kernel():
     for k in range(nzz):
         assert np.array_equal(Ug[:, k], Ug[:, 0])          # every plane the same bits
     assert max(rel_l1_fields(Ug[:, :1], Uo)) <= TOL[MIXED]
+
+
+# --------------------------------------------------------------------------- Sec. 3.3 van Leer integrator (reading S15)
+VL = binding.INTEGRATOR_VANLEER
+CASES_VL = [((45, 19, 23), (P, P, P, P, P, P)), ((37, 33, 10), (F, F, O, O, R, R)), ((64, 32, 8), (R, O, P, P, F, R)),
+            ((37, 21, 1), (P, P, P, P, P, P)), ((64, 48, 1), (R, R, O, F, P, P)), ((50, 1, 1), (F, F, P, P, P, P)),
+            ((1, 20, 22), (P, P, R, R, P, P))]
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("shape,bc", CASES_VL)
+def test_vanleer_parity(shape, bc, prec):
+    """Predictor kept as float_t primitives, corrector in place: element-wise against the
+    oracle's van Leer step with the oracle's dt sequence."""
+    nx, ny, nz = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=nx + ny + nz, gamma=1.4, bc=bc)
+    Uo = pr.U.copy()
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, integrator=VL)
+    h.set_state(pr.U)
+    for _ in range(5):
+        dt = oracle.cfl_dt(Uo, pr.gamma, 0.4)
+        oracle.step(Uo, pr.gamma, pr.bc, dt, integrator=oracle.VANLEER)
+        h.step(dt)
+    Ug = h.get_state()
+    assert h.floor_hits() == 0
+    h.destroy()
+    err = rel_l1_fields(Ug, Uo)
+    assert max(err) <= TOL[prec], err
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_vanleer_run_conservation_and_fixed_point(prec):
+    # device-resident dt (run) against the oracle's run, and conservation "up to the full machine accuracy" (PAPER.md:274)
+    pr = inputs.turbulence_3d(32, seed=7, nsteps=20)
+    Uo = pr.U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 20, integrator=oracle.VANLEER)
+    h = binding.KratosHydro(32, 32, 32, pr.gamma, pr.bc, precision=prec, integrator=VL)
+    h.set_state(pr.U)
+    T0 = h.totals()
+    A0 = np.array([math.fsum(np.abs(pr.U[m]).ravel()) for m in range(5)])
+    h.run(0.4, 20)
+    T1 = h.totals()
+    Ug = h.get_state()
+    h.destroy()
+    assert max(rel_l1_fields(Ug, Uo)) <= TOL[prec]
+    assert (np.abs(T1 - T0) / np.maximum(np.abs(T0), A0)).max() <= 1e-13
+    # uniform state: bitwise fixed point
+    U0 = np.ascontiguousarray(inputs.prim_to_cons(np.full((12, 20, 40), 1.3), 0.7, 0.4, -1.1, 2.2, 1.4))
+    h = binding.KratosHydro(40, 20, 12, 1.4, (P,) * 6, precision=prec, integrator=VL)
+    h.set_state(U0)
+    for _ in range(3):
+        h.step(1e-3)
+    np.testing.assert_array_equal(h.get_state(), U0)
+    h.destroy()
+
+
+def test_vanleer_refuses_the_heun_stage_kernels_and_bad_scheme_words():
+    pr = inputs.random_smooth(64, 32, 8, seed=1)
+    h = binding.KratosHydro(64, 32, 8, pr.gamma, pr.bc, precision=MIXED, integrator=VL)
+    for k in (TILED, PAIRED, ROLES, TMA):
+        with pytest.raises(Exception):
+            h.set_kernel(k)
+    h.destroy()
+    with pytest.raises(Exception):
+        binding.KratosHydro(64, 32, 8, pr.gamma, pr.bc, precision=MIXED, integrator=2 << 4)
