@@ -33,6 +33,8 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/sec per B200 (3D hydro step) and % of HBM roofline"
 UNIT = "cell-updates/s"
 BYTES_PER_CELL = {"stage1": 80.0, "stage2": 120.0}  # algorithmic HBM bytes per cell
+# van Leer, mixed precision: predictor 40 B read + 20 B written, corrector 20 + 40 read + 40 written
+BYTES_PER_CELL_VL = {"stage1": 60.0, "stage2": 100.0}
 
 
 def workload(name: str):
@@ -200,7 +202,13 @@ def run_ours(args):
     stream = torch.cuda.Stream()
     variant = {"auto": binding.KERNEL_AUTO, "simple": binding.KERNEL_SIMPLE, "tiled": binding.KERNEL_TILED,
                "paired": binding.KERNEL_PAIRED, "roles": binding.KERNEL_ROLES, "tma": binding.KERNEL_TMA}[args.kernel]
-    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream, kernel=variant)
+    vanleer = args.integrator == "vanleer"
+    bpc = dict(BYTES_PER_CELL)
+    if vanleer:
+        bpc = dict(BYTES_PER_CELL_VL) if prec == binding.PREC_MIXED else {"stage1": 80.0, "stage2": 120.0}
+    step_bytes = bpc["stage1"] + bpc["stage2"]
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, stream=stream, kernel=variant,
+                            integrator=binding.INTEGRATOR_VANLEER if vanleer else binding.INTEGRATOR_HEUN)
     if args.zchunk > 0:
         h.set_zchunk(args.zchunk)
     host = torch.from_numpy(pr.U).pin_memory()            # pinned host copy (e2e leg)
@@ -268,18 +276,20 @@ def run_ours(args):
         tot_ms, n = timing[k]
         if n:
             avg = tot_ms / n
-            gbs = BYTES_PER_CELL[k] * ncell / (avg * 1e-3) / 1e9
-            kern[k] = {"avg_ms": avg, "launches": n, "algorithmic_bytes": BYTES_PER_CELL[k] * ncell,
+            gbs = bpc[k] * ncell / (avg * 1e-3) / 1e9
+            kern[k] = {"avg_ms": avg, "launches": n, "algorithmic_bytes": bpc[k] * ncell,
                        "achieved_gbs": gbs, "frac": gbs / peak}
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
         kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel, (nx, ny, nz))
+        if vanleer:
+            kname = ("vl::predict<%s>" if dom == "stage1" else "vl::correct<%s>") % ("float" if prec == 0 else "double")
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                     "unit": "GB/s", "frac": kern[dom]["frac"],
                     "traffic": ncu_traffic(args.workload, args.precision, kname),
-                    "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL[dom]}
-    step_frac = value / world * 200.0 / (peak * 1e9)
+                    "peak_source": peak_src, "bytes_per_cell": bpc[dom]}
+    step_frac = value / world * step_bytes / (peak * 1e9)
 
     # ---- oracle on the host cores, bounded sample (rank 0, N = 1 only) ---------------------------
     cpu = None
@@ -295,7 +305,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32 flux / f64 state" if prec == 0 else "f64", "data": "synthetic",
         "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": args.precision,
-                   "scheme": "PLM-minmod + HLLC + Heun", "kernel": args.kernel, "cfl": pr.cfl, "parallelism": f"replicas x{world}",
+                   "scheme": "PLM-minmod + HLLC + " + ("van Leer" if vanleer else "Heun"), "kernel": args.kernel, "cfl": pr.cfl, "parallelism": f"replicas x{world}",
                    "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
                    if 40 * ncell > 2.5e8 else "state fits L2: no flush between steps (steps are data-dependent)",
                    "floor_hits": hits},
@@ -322,6 +332,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "roles", "tma"],
                     help="stage kernel variant (default: the library's own choice)")
+    ap.add_argument("--integrator", default="heun", choices=["heun", "vanleer"],
+                    help="time integrator (PAPER.md Sec. 3.3); the headline metric is quoted on heun")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per slab of the marching kernels (0 = auto)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
