@@ -119,6 +119,7 @@ void collect_timing(kratos_hydro* h)
 
 int auto_variant(const kratos_hydro* h)
 {
+    if (h->integ == 1) return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;  // van Leer
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
     if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
@@ -167,7 +168,10 @@ int launch_both_stages(kratos_hydro* h)
     if (h->integ == 1) {  // van Leer: predictor into the float_t primitive array, corrector in place
         for (int which = 1; which <= 2; which++) {
             LaunchTimer lt(h, which == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
-            if (h->prec == KRATOS_PREC_MIXED) vl::launch_step<float>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
+            if (which == 1 && h->maps && h->maps->ok && h->variant == KRATOS_KERNEL_TMA)   // predictor on the TMA machinery
+                tma::launch_vl_predict(*h->maps, h->g, h->ctrl,
+                                       h->zchunk > 0 ? (h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2]) : tma::auto_zchunk(h->g), h->stream);
+            else if (h->prec == KRATOS_PREC_MIXED) vl::launch_step<float>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
             else                              vl::launch_step<double>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
             cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "van Leer sub-step %d launch: %s", which, cudaGetErrorString(e));
@@ -309,9 +313,10 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     pr::configure();
     rl::configure();
     tma::configure();
-    if (prec == KRATOS_PREC_MIXED && integ == 0 && tma::supported(g)) {
+    if (prec == KRATOS_PREC_MIXED && tma::supported(g)) {
         h->maps = new (std::nothrow) tma::StageMaps;
-        if (h->maps) tma::build_maps(h->maps, h->U0, h->U1, g);
+        if (h->maps && integ == 0) tma::build_maps(h->maps, h->U0, h->U1, g);
+        if (h->maps && integ == 1) tma::build_maps_vl(h->maps, h->U0, (const float*)h->U1, g);
     }
     h->variant = auto_variant(h);
     return h;

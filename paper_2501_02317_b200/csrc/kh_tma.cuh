@@ -293,17 +293,29 @@ __device__ __forceinline__ void from_normal(const f2 F[5], f2 Fo[5])
 
 // One Heun stage.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin + dt L(Uin))
 // (Uout aliases U0) and the CFL rate maximum of Uout.  3D only.
-template <int STAGE>
+// Face states of a cell: Eq. 3 slopes (MODE 0) or piecewise-constant states (MODE 1, van Leer predictor).
+template <int MODE>
+__device__ __forceinline__ void plm_m(f2 qm, f2 q, f2 qp, f2& qL, f2& qR)
+{
+    if (MODE == 1) { qL = q; qR = q; }
+    else plm(qm, q, qp, qL, qR);
+}
+
+// MODE 0: Heun stage.  MODE 1 (with STAGE 1): predictor of the van Leer integrator (Sec. 3.3, reading
+// S15): piecewise-constant face states (all slopes zero), half a time step, and the result leaves as float_t
+// primitives W^{n+1/2} = prim(U + dt/2 L_1(U)) (a float box written over the consumed raw plane and stored by TMA).
+template <int STAGE, int MODE = 0>
 __global__ void __launch_bounds__(NTHREADS, BLOCKS_PER_SM)
 stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
+    static_assert(MODE == 0 || STAGE == 1, "the van Leer predictor has the data flow of stage 1");
     using S = Smem<STAGE>;
     constexpr int NSLOT = S::NSLOT;
     constexpr int NHALO = S::NHALO;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     S& sm = *reinterpret_cast<S*>(smem_raw);
 
-    const double dt = ctrl->dt;
+    const double dt = (MODE == 1) ? 0.5 * ctrl->dt : ctrl->dt;
     if (!(dt > 0.0)) return;  // a step clipped to zero length (run_until past t_end) does nothing
     const double pref_d = ctrl->p_ref;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -383,7 +395,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
             for (int f = 0; f < 5; f++) {
                 f2 qR;
-                plm(Wm[f], Wa[f], Wb[f], QLz[f], qR);
+                plm_m<MODE>(Wm[f], Wa[f], Wb[f], QLz[f], qR);
                 Fzlo[f] = make_double2(0.0, 0.0);
             }
         }
@@ -415,7 +427,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                     for (int f = 0; f < 5; f++) {
                         qL[f] = QLz[f];
-                        plm(Wa[f], Wb[f], Wn[f], QLz[f], qR[f]);
+                        plm_m<MODE>(Wa[f], Wb[f], Wn[f], QLz[f], qR[f]);
                     }
                     to_normal<2>(qL, L[0]);
                     to_normal<2>(qR, R[0]);
@@ -540,15 +552,31 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     const f2 q = Wb[f];  // W(k+1)
-                    plm(xm[f], q, xp[f], qLx[f], QRx[f]);
-                    plm(mk(below[f], q.x), q, mk(q.y, above[f]), qLy[f], QRy[f]);
+                    plm_m<MODE>(xm[f], q, xp[f], qLx[f], QRx[f]);
+                    plm_m<MODE>(mk(below[f], q.x), q, mk(q.y, above[f]), qLy[f], QRy[f]);
                     QLyo[f] = qLy[f].x;
                 }
                 KH_PROBE(5)
+                if (MODE == 1) {
+                    // W^{n+1/2} as float_t primitives (actual pressure: offset 0), written as a float box [5][PTY][PTX]
+                    // over the head of the raw plane just consumed (every thread read its entries before barrier 2)
+                    float Wpa[5], Wpb[5];
+                    const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, 0.0, VN_KEEP, VN_KEEP, VN_KEEP, Wpa);
+                    const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, 0.0, VN_KEEP, VN_KEEP, VN_KEEP, Wpb);
+                    if (live) hits += ha + hb;
+                    float* const sf = reinterpret_cast<float*>(raw0 + s_upd * RAWS - (2 * w * PTX + lane)) + (2 * w * PTX + lane);
+#pragma unroll
+                    for (int f = 0; f < 5; f++) {
+                        sf[f * RAWF] = Wpa[f];
+                        sf[f * RAWF + PTX] = Wpb[f];
+                    }
+                }
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    su[f * RAWF] = ua[f];
-                    su[f * RAWF + PTX] = ub[f];
+                    if (MODE == 0) {
+                        su[f * RAWF] = ua[f];
+                        su[f * RAWF + PTX] = ub[f];
+                    }
                     qlx[f * QXF + 1] = qLx[f];
                     qly[f * QYF + PTX] = qLy[f].y;
                 }
@@ -598,7 +626,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     // -> right state of the tile's high y face
                     const float qm = top ? nb[f].y : W0[f], q = top ? W0[f] : W1[f], qp = top ? W1[f] : nb[f].x;
                     f2 qL, qR;
-                    plm(mk(qm, qm), mk(q, q), mk(qp, qp), qL, qR);
+                    plm_m<MODE>(mk(qm, qm), mk(q, q), mk(qp, qp), qL, qR);
                     if (top) sm.QRyT[f][lane] = qR.x;
                     else     sm.QLy[f][0][lane] = qL.x;
                 }
@@ -682,7 +710,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) { wl[f] = wt[f * WTF + dl]; wr[f] = wt[f * WTF + dr]; }
 #pragma unroll
-                for (int f = 0; f < 5; f++) plm(wl[f], W[f], wr[f], qL[f], qR[f]);
+                for (int f = 0; f < 5; f++) plm_m<MODE>(wl[f], W[f], wr[f], qL[f], qR[f]);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     if (cid == 1 && xact) sm.QLx[f][rp][0] = qL[f];   // column -1: left state of the tile's low x face
@@ -832,6 +860,20 @@ inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx, int
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Tensor map over a float_t primitive array W[5][nz][ny][nx] (van Leer predictor output), box PTX x PTY x 1 x 5.
+inline bool make_map_f32(CUtensorMap* m, const float* W, const Grid& g)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2], 5};
+    const cuuint64_t strides[3] = {(cuuint64_t)g.n[0] * 4, (cuuint64_t)g.n[0] * g.n[1] * 4, (cuuint64_t)g.N * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)PTX, (cuuint32_t)PTY, 1, 5};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)W, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // maps of both stages for the two state buffers of a handle: stage 1 reads A writes B, stage 2 reads B, averages with
 // and writes A.
 struct StageMaps {
@@ -858,6 +900,26 @@ inline void build_maps(StageMaps* sm, const double* A, const double* B, const Gr
     sm->ok = true;
 }
 
+// van Leer: the predictor reads the state A and writes the float_t primitives Wh (maps in sm->s1; s2 unused)
+inline void build_maps_vl(StageMaps* sm, const double* A, const float* Wh, const Grid& g)
+{
+    sm->ok = false;
+    if (!supported(g) || (g.N * 4) % 16 != 0) return;
+    CUtensorMap a_own, a_rows, a_cols, w_own;
+    if (!make_map(&a_own, A, g, PTX, PTY) || !make_map(&a_rows, A, g, PTX, 2) || !make_map(&a_cols, A, g, 2, PTY) ||
+        !make_map_f32(&w_own, Wh, g))
+        return;
+    sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = w_own;
+    sm->s2 = sm->s1;
+    sm->ok = true;
+}
+
+inline void launch_vl_predict(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
+{
+    dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
+    stage_tma<1, 1><<<grid, NTHREADS, sizeof(Smem<1>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
+}
+
 inline int auto_zchunk(const Grid& g)
 {
     // >= ~6 waves of thread blocks over the 148 SMs (the tail of the last wave costs ~1 %), slabs of >= 32 planes
@@ -875,6 +937,8 @@ inline void configure()
                   "tile does not fit the shared memory of one SM");
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
+    cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
 }
