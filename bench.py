@@ -285,6 +285,8 @@ def run_ours(args):
         kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel, (nx, ny, nz))
         if vanleer:
             kname = ("vl::predict<%s>" if dom == "stage1" else "vl::correct<%s>") % ("float" if prec == 0 else "double")
+            if prec == 0 and nz > 1 and nx % 32 == 0 and ny % 16 == 0 and args.kernel in ("auto", "tma"):
+                kname = "stage_tma<1,1>" if dom == "stage1" else "stage_tma<2,2>"
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                     "unit": "GB/s", "frac": kern[dom]["frac"],
                     "traffic": ncu_traffic(args.workload, args.precision, kname),

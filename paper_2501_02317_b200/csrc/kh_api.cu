@@ -168,9 +168,10 @@ int launch_both_stages(kratos_hydro* h)
     if (h->integ == 1) {  // van Leer: predictor into the float_t primitive array, corrector in place
         for (int which = 1; which <= 2; which++) {
             LaunchTimer lt(h, which == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
-            if (which == 1 && h->maps && h->maps->ok && h->variant == KRATOS_KERNEL_TMA)   // predictor on the TMA machinery
-                tma::launch_vl_predict(*h->maps, h->g, h->ctrl,
-                                       h->zchunk > 0 ? (h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2]) : tma::auto_zchunk(h->g), h->stream);
+            const int zc = h->zchunk > 0 ? (h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2]) : tma::auto_zchunk(h->g);
+            const bool on_tma = h->maps && h->maps->ok && h->variant == KRATOS_KERNEL_TMA;   // both sub-steps on the TMA machinery
+            if (on_tma && which == 1) tma::launch_vl_predict(*h->maps, h->g, h->ctrl, zc, h->stream);
+            else if (on_tma && which == 2) tma::launch_vl_correct(*h->maps, h->g, h->ctrl, zc, h->stream);
             else if (h->prec == KRATOS_PREC_MIXED) vl::launch_step<float>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
             else                              vl::launch_step<double>(h->U0, h->U1, h->g, h->ctrl, h->stream, which);
             cudaError_t e = cudaGetLastError();

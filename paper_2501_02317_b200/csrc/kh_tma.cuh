@@ -170,13 +170,14 @@ __device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "me
 struct HaloSide {
     int start, idx0, idx1, rule;
 };
-__device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_hi)
+__device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_hi, int width = 2)
 {
     int r0, r1;
     const int s0 = bc_source(c0, n, bc_lo, bc_hi, r0);
     const int s1 = bc_source(c0 + 1, n, bc_lo, bc_hi, r1);
     HaloSide h;
-    h.start = min(s0, s1) & ~1;  // even: the box stays inside the block and its first byte 16-byte aligned
+    h.start = min(s0, s1) & ~(width - 1);  // aligned: the box stays inside the block, its first byte 16-byte aligned
+                                           // (width 2 for fp64 boxes, 4 for the float boxes of the van Leer corrector)
     h.idx0 = s0 - h.start;
     h.idx1 = s1 - h.start;
     h.rule = r0;  // both cells lie beyond the same face
@@ -304,11 +305,14 @@ __device__ __forceinline__ void plm_m(f2 qm, f2 q, f2 qp, f2& qL, f2& qR)
 // MODE 0: Heun stage.  MODE 1 (with STAGE 1): predictor of the van Leer integrator (Sec. 3.3, reading
 // S15): piecewise-constant face states (all slopes zero), half a time step, and the result leaves as float_t
 // primitives W^{n+1/2} = prim(U + dt/2 L_1(U)) (a float box written over the consumed raw plane and stored by TMA).
+// MODE 2 (with STAGE 2): its corrector U^{n+1} = U^n + dt L_2(W^{n+1/2}): the plane ring and the halo boxes carry the
+// float_t primitives (no recovery, no fp64 chain), U^n arrives through the U0 ring, is updated in place there and stored.
 template <int STAGE, int MODE = 0>
 __global__ void __launch_bounds__(NTHREADS, BLOCKS_PER_SM)
 stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
-    static_assert(MODE == 0 || STAGE == 1, "the van Leer predictor has the data flow of stage 1");
+    static_assert(MODE == 0 || (MODE == 1 && STAGE == 1) || (MODE == 2 && STAGE == 2),
+                  "the van Leer predictor has the data flow of stage 1, the corrector that of stage 2");
     using S = Smem<STAGE>;
     constexpr int NSLOT = S::NSLOT;
     constexpr int NHALO = S::NHALO;
@@ -371,6 +375,15 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             int rz = VN_KEEP;
             if (kk < 0 || kk >= nz) (void)bc_source(kk, nz, g.bc[4], g.bc[5], rz);
             mbar_wait_parity(&sm.full_raw[slot], parity);
+            if (MODE == 2) {  // the ring slot holds a float box [5][PTY][PTX] of primitives (rho, p, vx, vy, vz)
+                const float* sf = reinterpret_cast<const float*>(raw0 + slot * RAWS - (2 * w * PTX + lane)) + (2 * w * PTX + lane);
+                const float pref_f = (float)pref_d;
+#pragma unroll
+                for (int f = 0; f < 5; f++) W[f] = mk(sf[f * RAWF], sf[f * RAWF + PTX]);
+                W[1] = mk(__fadd_rn(W[1].x, -pref_f), __fadd_rn(W[1].y, -pref_f));
+                W[4] = mk(apply_vn_rule(W[4].x, rz), apply_vn_rule(W[4].y, rz));
+                return;
+            }
             const double* s = raw0 + slot * RAWS;
             double ua[5], ub[5];
 #pragma unroll
@@ -482,8 +495,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             double ua[5], ub[5], va[5], vb[5];
 #pragma unroll
             for (int f = 0; f < 5; f++) {
-                ua[f] = su[f * RAWF];
-                ub[f] = su[f * RAWF + PTX];
+                if (MODE != 2) {
+                    ua[f] = su[f * RAWF];
+                    ub[f] = su[f * RAWF + PTX];
+                }
                 if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
             }
             KH_PROBE(3)
@@ -516,9 +531,11 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 KH_PROBE(4)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    double xa = __dadd_rn(ua[f], __fma_rn(-dtdx, (double)fxh[f].x, dU[f].x));
-                    double xb = __dadd_rn(ub[f], __fma_rn(-dtdy, (double)fyh[f], __fma_rn(-dtdx, (double)fxh[f].y, dU[f].y)));
-                    if (STAGE == 2) {
+                    // the state the flux differences are added to: the stage input (Heun), U^n (van Leer corrector)
+                    const double ba = (MODE == 2) ? va[f] : ua[f], bb = (MODE == 2) ? vb[f] : ub[f];
+                    double xa = __dadd_rn(ba, __fma_rn(-dtdx, (double)fxh[f].x, dU[f].x));
+                    double xb = __dadd_rn(bb, __fma_rn(-dtdy, (double)fyh[f], __fma_rn(-dtdx, (double)fxh[f].y, dU[f].y)));
+                    if (STAGE == 2 && MODE == 0) {
                         xa = __fma_rn(0.5, va[f], __dmul_rn(0.5, xa));
                         xb = __fma_rn(0.5, vb[f], __dmul_rn(0.5, xb));
                     }
@@ -576,6 +593,11 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     if (MODE == 0) {
                         su[f * RAWF] = ua[f];
                         su[f * RAWF + PTX] = ub[f];
+                    }
+                    if (MODE == 2 && live) {  // U^{n+1} over U^n in the U0 ring: the producer ships that box
+                        double* const sv = const_cast<double*>(s0);
+                        sv[f * RAWF] = ua[f];
+                        sv[f * RAWF + PTX] = ub[f];
                     }
                     qlx[f * QXF + 1] = qLx[f];
                     qly[f * QYF + PTX] = qLy[f].y;
@@ -669,11 +691,20 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             if (k + 1 < kend) {
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = h0 + hs * HSLOT;
+                if (MODE == 2) {  // float primitives: [side][field][box row][column], 1280 bytes per side
+                    const float* sf = reinterpret_cast<const float*>(s) + (top ? 5 * 2 * PTX : 0) + lane;
+                    const float pref_f = (float)pref_d;
+#pragma unroll
+                    for (int f = 0; f < 5; f++) { W0[f] = sf[f * 2 * PTX + hsd.idx0 * PTX]; W1[f] = sf[f * 2 * PTX + hsd.idx1 * PTX]; }
+                    W0[1] = __fadd_rn(W0[1], -pref_f); W1[1] = __fadd_rn(W1[1], -pref_f);
+                    W0[3] = apply_vn_rule(W0[3], ry);  W1[3] = apply_vn_rule(W1[3], ry);
+                } else {
                 double u0[5], u1[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) { u0[f] = s[off0 + f * HF]; u1[f] = s[off1 + f * HF]; }
                 (void)recover(u0[0], u0[1], u0[2], u0[3], u0[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W0);
                 (void)recover(u1[0], u1[1], u1[2], u1[3], u1[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W1);
+                }
 #pragma unroll
                 for (int f = 0; f < 5; f++) wown[f * WTF] = mk(W0[f], W1[f]);
                 if (++hs == NHALO) { hs = 0; hpar ^= 1u; }
@@ -686,7 +717,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         const int cid = lane & 3, rp = min(lane >> 2, PRP - 1);     // column id, row pair
         const bool xact = (lane >> 2) < PRP;                        // (a tile of 8 rows keeps half the lanes busy)
         const int col = (cid < 2) ? cid - 2 : PTX + cid - 2;
-        const HaloSide side = (cid < 2) ? halo_side(i0 - 2, nx, g.bc[0], g.bc[1]) : halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
+        constexpr int XW = (MODE == 2) ? 4 : 2;   // width of the halo column boxes (16 bytes: 2 doubles or 4 floats)
+        const HaloSide side = (cid < 2) ? halo_side(i0 - 2, nx, g.bc[0], g.bc[1], XW) : halo_side(i0 + PTX, nx, g.bc[0], g.bc[1], XW);
         const int bidx = (cid & 1) ? side.idx1 : side.idx0;
         const int rx = side.rule;
         constexpr int CF = PTY * 2, CSIDE = 5 * CF, CSLOT = 2 * CSIDE;   // double strides of hcol: field, side, slot
@@ -722,12 +754,22 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             if (k + 1 < kend) {
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = c0 + hs * CSLOT;
+                float Wa[5], Wb[5];
+                if (MODE == 2) {  // float primitives: [side][field][row][box column], 4 columns per box, 1280 bytes per side
+                    const float* sf = reinterpret_cast<const float*>(&sm.hcol[0][0][0][0][0] + hs * CSLOT) +
+                                      (cid >> 1) * (5 * PTY * 4) + (2 * rp) * 4 + bidx;
+                    const float pref_f = (float)pref_d;
+#pragma unroll
+                    for (int f = 0; f < 5; f++) { Wa[f] = sf[f * PTY * 4]; Wb[f] = sf[f * PTY * 4 + 4]; }
+                    Wa[1] = __fadd_rn(Wa[1], -pref_f); Wb[1] = __fadd_rn(Wb[1], -pref_f);
+                    Wa[2] = apply_vn_rule(Wa[2], rx);  Wb[2] = apply_vn_rule(Wb[2], rx);
+                } else {
                 double ua[5], ub[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) { ua[f] = s[f * CF]; ub[f] = s[f * CF + 2]; }
-                float Wa[5], Wb[5];
                 (void)recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wa);
                 (void)recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wb);
+                }
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     W[f] = mk(Wa[f], Wb[f]);
@@ -742,23 +784,31 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         // ================================ producer warp: all global traffic, by TMA =====================
         const HaloSide ylo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
         const HaloSide yhi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
-        const HaloSide xlo = halo_side(i0 - 2, nx, g.bc[0], g.bc[1]);
-        const HaloSide xhi = halo_side(i0 + PTX, nx, g.bc[0], g.bc[1]);
+        constexpr int XW = (MODE == 2) ? 4 : 2;                        // halo column boxes: 2 doubles or 4 floats wide
+        constexpr unsigned RAW_TX = (MODE == 2) ? OWN_BYTES / 2 : OWN_BYTES;   // float primitives are half the bytes
+        constexpr unsigned HALO_TX = (MODE == 2) ? 4 * 1280 : 2 * ROW_BYTES + 2 * COL_BYTES;
+        const HaloSide xlo = halo_side(i0 - 2, nx, g.bc[0], g.bc[1], XW);
+        const HaloSide xhi = halo_side(i0 + PTX, nx, g.bc[0], g.bc[1], XW);
         const int plast = kend + 2;  // planes up to kend+1 feed the z stencil; the main warps convert one plane further
                                      // (unconditionally: straight-line code), so that one is loaded too
         auto load_raw = [&](int p, int slot) {
             int rz;
             const int sk = bc_source(p, nz, g.bc[4], g.bc[5], rz);
-            mbar_expect_tx(&sm.full_raw[slot], OWN_BYTES);
+            mbar_expect_tx(&sm.full_raw[slot], RAW_TX);
             tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);
         };
         auto load_halo = [&](int p, int slot) {  // p in [kbeg, kend): an interior plane
             unsigned long long* bar = &sm.full_halo[slot];
-            mbar_expect_tx(bar, 2 * ROW_BYTES + 2 * COL_BYTES);
+            mbar_expect_tx(bar, HALO_TX);
+            // second side of each pair: right behind the first one (float boxes are 1280 bytes each)
+            char* const r1 = (MODE == 2) ? reinterpret_cast<char*>(&sm.hrow[slot][0][0][0][0]) + 1280
+                                         : reinterpret_cast<char*>(&sm.hrow[slot][1][0][0][0]);
+            char* const c1 = (MODE == 2) ? reinterpret_cast<char*>(&sm.hcol[slot][0][0][0][0]) + 1280
+                                         : reinterpret_cast<char*>(&sm.hcol[slot][1][0][0][0]);
             tma_load4(&sm.hrow[slot][0][0][0][0], &maps.in_rows, i0, ylo.start, p, 0, bar);
-            tma_load4(&sm.hrow[slot][1][0][0][0], &maps.in_rows, i0, yhi.start, p, 0, bar);
+            tma_load4(r1, &maps.in_rows, i0, yhi.start, p, 0, bar);
             tma_load4(&sm.hcol[slot][0][0][0][0], &maps.in_cols, xlo.start, j0, p, 0, bar);
-            tma_load4(&sm.hcol[slot][1][0][0][0], &maps.in_cols, xhi.start, j0, p, 0, bar);
+            tma_load4(c1, &maps.in_cols, xhi.start, j0, p, 0, bar);
         };
         if (lane == 0) {
             for (int q = 0; q < NSLOT; q++)
@@ -772,7 +822,23 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         for (int k = kfirst; k < kend; k++) {
             __syncwarp();
             block_bar();
-            if (lane == 0) {
+            if (MODE == 2 && lane == 0) {
+                // van Leer corrector: the primitive planes are only read, U^n is updated in place in the U0 ring
+                const bool stored = k - 1 >= kbeg;
+                if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
+                if (k - 1 + NSLOT <= plast) load_raw(k - 1 + NSLOT, s_prev);
+                if (stored) {
+                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.u0[(k - 1 - kbeg) & 1][0][0][0]);
+                    tma_commit();
+                }
+                if (k + 1 < kend) {
+                    const int m = (k + 1 - kbeg) & 1;
+                    if (stored) tma_wait_read0();  // plane k-1 left this slot
+                    mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
+                    tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
+                }
+            }
+            if (MODE != 2 && lane == 0) {
                 const bool stored = k - 1 >= kbeg;
                 if (stored) {  // plane k-1 was updated in place in phase C of the previous iteration
                     tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.raw[s_prev][0][0][0]);
@@ -786,7 +852,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 }
             }
             __syncwarp();
-            if (lane == 0) {  // refill the slot the store is reading from
+            if (MODE != 2 && lane == 0) {  // refill the slot the store is reading from
                 const bool stored = k - 1 >= kbeg;
                 const int p = k - 1 + NSLOT;
                 if (p <= plast) {
@@ -802,7 +868,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         __syncwarp();
         block_bar();
         if (lane == 0) {  // the last plane of the slab
-            tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.raw[s_prev][0][0][0]);
+            if (MODE == 2) tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.u0[(kend - 1 - kbeg) & 1][0][0][0]);
+            else           tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.raw[s_prev][0][0][0]);
             tma_commit();
             tma_wait_all0();
         }
@@ -860,14 +927,14 @@ inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx, int
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Tensor map over a float_t primitive array W[5][nz][ny][nx] (van Leer predictor output), box PTX x PTY x 1 x 5.
-inline bool make_map_f32(CUtensorMap* m, const float* W, const Grid& g)
+// Tensor map over a float_t primitive array W[5][nz][ny][nx] (van Leer predictor output), box bx x by x 1 x 5.
+inline bool make_map_f32(CUtensorMap* m, const float* W, const Grid& g, int bx = PTX, int by = PTY)
 {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
     const cuuint64_t dims[4] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2], 5};
     const cuuint64_t strides[3] = {(cuuint64_t)g.n[0] * 4, (cuuint64_t)g.n[0] * g.n[1] * 4, (cuuint64_t)g.N * 4};
-    const cuuint32_t box[4] = {(cuuint32_t)PTX, (cuuint32_t)PTY, 1, 5};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 5};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)W, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -905,13 +972,20 @@ inline void build_maps_vl(StageMaps* sm, const double* A, const float* Wh, const
 {
     sm->ok = false;
     if (!supported(g) || (g.N * 4) % 16 != 0) return;
-    CUtensorMap a_own, a_rows, a_cols, w_own;
+    CUtensorMap a_own, a_rows, a_cols, w_own, w_rows, w_cols;
     if (!make_map(&a_own, A, g, PTX, PTY) || !make_map(&a_rows, A, g, PTX, 2) || !make_map(&a_cols, A, g, 2, PTY) ||
-        !make_map_f32(&w_own, Wh, g))
+        !make_map_f32(&w_own, Wh, g) || !make_map_f32(&w_rows, Wh, g, PTX, 2) || !make_map_f32(&w_cols, Wh, g, 4, PTY))
         return;
     sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = w_own;
-    sm->s2 = sm->s1;
+    // corrector: primitive planes and halo boxes from Wh (columns 4 floats = 16 bytes wide), U^n in and out through A
+    sm->s2.in_own = w_own; sm->s2.in_rows = w_rows; sm->s2.in_cols = w_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
     sm->ok = true;
+}
+
+inline void launch_vl_correct(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
+{
+    dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
+    stage_tma<2, 2><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
 }
 
 inline void launch_vl_predict(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
@@ -937,6 +1011,8 @@ inline void configure()
                   "tile does not fit the shared memory of one SM");
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<2, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
