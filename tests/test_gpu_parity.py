@@ -544,3 +544,22 @@ def test_vanleer_refuses_the_heun_stage_kernels_and_bad_scheme_words():
     h.destroy()
     with pytest.raises(Exception):
         binding.KratosHydro(64, 32, 8, pr.gamma, pr.bc, precision=MIXED, integrator=2 << 4)
+
+
+@pytest.mark.parametrize("zchunk", [1, 3, 8, 1000])
+def test_vanleer_tma_slab_seams_and_general_kernels_agree(zchunk):
+    """van Leer on the TMA kernel: slabs of any height give the same bits, and the result agrees with the general
+    one-thread-per-cell kernels to float_t rounding of the stored predictor."""
+    pr = inputs.random_smooth(64, 32, 21, seed=8, gamma=1.4, bc=(R, O, P, P, F, R))
+    outs = []
+    for kern, zc in ((TMA, zchunk), (TMA, 21), (SIMPLE, 0)):
+        h = binding.KratosHydro(64, 32, 21, pr.gamma, pr.bc, precision=MIXED, integrator=VL, kernel=kern)
+        if zc:
+            h.set_zchunk(zc)
+        h.set_state(pr.U)
+        for _ in range(3):
+            h.step(2e-3)
+        outs.append(h.get_state())
+        h.destroy()
+    np.testing.assert_array_equal(outs[0], outs[1])
+    assert max(rel_l1_fields(outs[0], outs[2])) <= 1e-6
