@@ -78,12 +78,16 @@ constexpr int OWN_BYTES = 5 * PTY * PTX * 8;    // one tile box
 constexpr int ROW_BYTES = 5 * 2 * PTX * 8;      // one halo row pair
 constexpr int COL_BYTES = 5 * PTY * 2 * 8;      // one halo column pair
 
-template <int STAGE>
+template <int STAGE, int MODE = 0>
 struct Smem {
     static constexpr int NSLOT = Cfg<STAGE>::NSLOT;
     static constexpr int NHALO = Cfg<STAGE>::NHALO;
-    alignas(128) double raw[NSLOT][5][PTY][PTX];              // fp64 state of the tile, planes in flight
-    alignas(128) double u0[(STAGE == 2) ? 2 : 1][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
+    // U0 ring: two planes for the Heun average; three for the van Leer corrector, which also stores from it (the
+    // refill of a slot then never waits for the store that is still reading the previous plane)
+    static constexpr int NU0 = (STAGE == 2) ? ((MODE == 2) ? 3 : 2) : 1;
+    // planes in flight: fp64 conserved state, or (van Leer corrector) float_t primitives = half the bytes
+    alignas(128) double raw[NSLOT][5][(MODE == 2) ? PTY / 2 : PTY][PTX];
+    alignas(128) double u0[NU0][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
     alignas(128) double hrow[NHALO][2][5][2][PTX];            // halo rows: [lo/hi][field][box row][column]
     alignas(128) double hcol[NHALO][2][5][PTY][2];            // halo columns: [lo/hi][field][row][box column]
     f2 Wt[5][PRP + 2][PTX + 4];                               // primitives of one plane, row pairs -1..PRP, columns -2..PTX+1
@@ -96,7 +100,7 @@ struct Smem {
     double red[32];
     unsigned long long full_raw[NSLOT];
     unsigned long long full_halo[NHALO];
-    unsigned long long full_u0[2];
+    unsigned long long full_u0[3];
 };
 
 // tensor maps of one stage launch (64-byte aligned kernel parameters)
@@ -313,7 +317,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
     static_assert(MODE == 0 || (MODE == 1 && STAGE == 1) || (MODE == 2 && STAGE == 2),
                   "the van Leer predictor has the data flow of stage 1, the corrector that of stage 2");
-    using S = Smem<STAGE>;
+    using S = Smem<STAGE, MODE>;
+    constexpr int NU0 = S::NU0;
     constexpr int NSLOT = S::NSLOT;
     constexpr int NHALO = S::NHALO;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -339,8 +344,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSLOT; s++) mbar_init(&sm.full_raw[s], 1);
         for (int s = 0; s < NHALO; s++) mbar_init(&sm.full_halo[s], 1);
-        mbar_init(&sm.full_u0[0], 1);
-        mbar_init(&sm.full_u0[1], 1);
+        for (int s = 0; s < 3; s++) mbar_init(&sm.full_u0[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -359,7 +363,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         constexpr int WTF = (PRP + 2) * (PTX + 4);                    // f2 field stride of Wt
         constexpr int QXF = PRP * (PTX + 1);                          // f2 field stride of QLx, double2 of Fx
         constexpr int QYF = (PRP + 1) * PTX;                          // field stride of QLy (float) and Fy (double)
-        double* const raw0 = &sm.raw[0][0][2 * w][lane];              // row 2w; row 2w+1 is + PTX
+        double* const raw0 = (MODE == 2) ? &sm.raw[0][0][0][0]        // (float planes: addressed in convert)
+                                         : &sm.raw[0][0][2 * w][lane]; // row 2w; row 2w+1 is + PTX
         const double* const u00 = &sm.u0[0][0][(STAGE == 2) ? 2 * w : 0][lane];
         f2* const wt = &sm.Wt[0][w + 1][lane + 2];
         f2* const qlx = &sm.QLx[0][w][lane];      // left state of the own low x face; own high face is + 1
@@ -376,7 +381,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             if (kk < 0 || kk >= nz) (void)bc_source(kk, nz, g.bc[4], g.bc[5], rz);
             mbar_wait_parity(&sm.full_raw[slot], parity);
             if (MODE == 2) {  // the ring slot holds a float box [5][PTY][PTX] of primitives (rho, p, vx, vy, vz)
-                const float* sf = reinterpret_cast<const float*>(raw0 + slot * RAWS - (2 * w * PTX + lane)) + (2 * w * PTX + lane);
+                const float* sf = reinterpret_cast<const float*>(&sm.raw[0][0][0][0]) + slot * RAWS + (2 * w * PTX + lane);
                 const float pref_f = (float)pref_d;
 #pragma unroll
                 for (int f = 0; f < 5; f++) W[f] = mk(sf[f * RAWF], sf[f * RAWF + PTX]);
@@ -490,8 +495,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             // The thread's own fp64 data for the update (nobody else touches these entries) are fetched BEFORE the barrier:
             // their latency hides behind the barrier wait and they stay out of the load burst that follows it.
             double* const su = raw0 + s_upd * RAWS;
-            const double* const s0 = u00 + ((k - kbeg) & 1) * RAWS;
-            if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[(k - kbeg) & 1], (unsigned)((k - kbeg) >> 1) & 1u);
+            const int m0 = max(k - kbeg, 0);
+            const double* const s0 = u00 + (m0 % NU0) * RAWS;
+            if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[m0 % NU0], (unsigned)(m0 / NU0) & 1u);
             double ua[5], ub[5], va[5], vb[5];
 #pragma unroll
             for (int f = 0; f < 5; f++) {
@@ -795,7 +801,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             int rz;
             const int sk = bc_source(p, nz, g.bc[4], g.bc[5], rz);
             mbar_expect_tx(&sm.full_raw[slot], RAW_TX);
-            tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);
+            tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);   // (slot stride follows the type)
         };
         auto load_halo = [&](int p, int slot) {  // p in [kbeg, kend): an interior plane
             unsigned long long* bar = &sm.full_halo[slot];
@@ -828,12 +834,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
                 if (k - 1 + NSLOT <= plast) load_raw(k - 1 + NSLOT, s_prev);
                 if (stored) {
-                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.u0[(k - 1 - kbeg) & 1][0][0][0]);
+                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.u0[(k - 1 - kbeg) % NU0][0][0][0]);
                     tma_commit();
                 }
                 if (k + 1 < kend) {
-                    const int m = (k + 1 - kbeg) & 1;
-                    if (stored) tma_wait_read0();  // plane k-1 left this slot
+                    const int m = (k + 1 - kbeg) % NU0;
+                    // this slot held plane k-2, whose store was committed one group before the one just issued
+                    if (stored) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
                     mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
                     tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
                 }
@@ -846,7 +853,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 }
                 if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
                 if (STAGE == 2 && k + 1 < kend) {
-                    const int m = (k + 1 - kbeg) & 1;
+                    const int m = (k + 1 - kbeg) % NU0;
                     mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
                     tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
                 }
@@ -868,7 +875,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         __syncwarp();
         block_bar();
         if (lane == 0) {  // the last plane of the slab
-            if (MODE == 2) tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.u0[(kend - 1 - kbeg) & 1][0][0][0]);
+            if (MODE == 2) tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.u0[(kend - 1 - kbeg) % NU0][0][0][0]);
             else           tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.raw[s_prev][0][0][0]);
             tma_commit();
             tma_wait_all0();
@@ -985,7 +992,7 @@ inline void build_maps_vl(StageMaps* sm, const double* A, const float* Wh, const
 inline void launch_vl_correct(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
 {
     dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
-    stage_tma<2, 2><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
+    stage_tma<2, 2><<<grid, NTHREADS, sizeof(Smem<2, 2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
 }
 
 inline void launch_vl_predict(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
@@ -1007,11 +1014,11 @@ inline int auto_zchunk(const Grid& g)
 inline void configure()
 {
     constexpr size_t per_block = (228 * 1024) / BLOCKS_PER_SM - 1024;
-    static_assert(sizeof(Smem<1>) + 128 <= per_block && sizeof(Smem<2>) + 128 <= per_block,
+    static_assert(sizeof(Smem<1>) + 128 <= per_block && sizeof(Smem<2>) + 128 <= per_block && sizeof(Smem<2, 2>) + 128 <= per_block,
                   "tile does not fit the shared memory of one SM");
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
-    cudaFuncSetAttribute(stage_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2, 2>) + 128);
     cudaFuncSetAttribute(stage_tma<2, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
