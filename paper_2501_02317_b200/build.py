@@ -52,7 +52,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed (exit %d)" % res.returncode)
     os.replace(tmp, LIB)
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+        # (the temporary output name carries the pid: log the final name so that rebuilding leaves the file unchanged)
+        f.write(" ".join(cmd).replace(tmp, LIB) + "\n" + (res.stdout + res.stderr).replace(tmp, LIB))
     return LIB
 
 
