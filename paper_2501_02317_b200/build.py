@@ -53,7 +53,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.replace(tmp, LIB)
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as f:
         # (the temporary output name carries the pid: log the final name so that rebuilding leaves the file unchanged)
-        f.write(" ".join(cmd).replace(tmp, LIB) + "\n" + (res.stdout + res.stderr).replace(tmp, LIB))
+        log = (res.stdout + res.stderr).replace(tmp, LIB)
+        log = "\n".join(l for l in log.split("\n") if "Compile time" not in l)
+        f.write(" ".join(cmd).replace(tmp, LIB) + "\n" + log)
     return LIB
 
 
