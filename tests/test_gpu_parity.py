@@ -563,3 +563,35 @@ def test_vanleer_tma_slab_seams_and_general_kernels_agree(zchunk):
         h.destroy()
     np.testing.assert_array_equal(outs[0], outs[1])
     assert max(rel_l1_fields(outs[0], outs[2])) <= 1e-6
+
+
+# --------------------------------------------------------------------------- seeded random blocks through the TMA kernels
+@pytest.mark.parametrize("integrator", ["heun", "vanleer"])
+def test_random_blocks_boundaries_spacings_and_slabs(integrator):
+    """Twelve seeded random combinations of extent (multiples of the 32 x 16 tile), boundary rules per face, cell
+    aspect ratio, gamma and slab height: the TMA kernels with the device-resident dt against the oracle's run."""
+    rng = np.random.default_rng(77 if integrator == "heun" else 78)
+    vl = integrator == "vanleer"
+    for it in range(12):
+        nx, ny, nz = 32 * int(rng.integers(1, 4)), 16 * int(rng.integers(1, 4)), int(rng.integers(4, 30))
+        bc = []
+        for _ in range(3):
+            bc += [0, 0] if rng.random() < 0.4 else [int(rng.integers(1, 4)), int(rng.integers(1, 4))]
+        zc = int(rng.choice([0, 1, 2, 3, 5, 7, 11, 16]))
+        pr = inputs.random_smooth(nx, ny, nz, seed=100 + it, gamma=float(rng.choice([1.4, 5 / 3, 1.1])), bc=tuple(bc))
+        sp = (1.0 / nx, float(rng.uniform(0.5, 2)) / ny, float(rng.uniform(0.5, 2)) / nz)
+        h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=MIXED, spacing=sp, kernel=TMA,
+                                integrator=VL if vl else binding.INTEGRATOR_HEUN)
+        if zc:
+            h.set_zchunk(zc)
+        h.set_state(pr.U)
+        T0 = h.totals()
+        h.run(0.4, 6)
+        Ug, T1, hits = h.get_state(), h.totals(), h.floor_hits()
+        h.destroy()
+        Uo = pr.U.copy()
+        oracle.run(Uo, pr.gamma, pr.bc, 0.4, 6, spacing=sp, integrator=oracle.VANLEER if vl else oracle.HEUN)
+        assert hits == 0 and np.isfinite(Ug).all()
+        assert max(rel_l1_fields(Ug, Uo)) <= TOL[MIXED], (it, (nx, ny, nz), bc, zc)
+        if all(b == 0 for b in bc):
+            assert abs(T1[0] - T0[0]) <= 1e-13 * abs(T0[0]) and abs(T1[4] - T0[4]) <= 1e-13 * abs(T0[4])
