@@ -59,7 +59,8 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
 #define KRATOS_INTEGRATOR_HEUN (0 << 4)
 #define KRATOS_INTEGRATOR_VANLEER (1 << 4) /* predictor-corrector of Sec. 3.3: predictor kept as float_t
                                              primitives (20 B per cell in mixed precision instead of a second fp64 state);
-                                             served by the general one-thread-per-cell kernels */
+                                             both sub-steps run on the TMA kernel where KRATOS_KERNEL_TMA applies, else on
+                                             general one-thread-per-cell kernels (KRATOS_KERNEL_SIMPLE) */
 
 /* boundary codes, the paper's list order */
 #define KRATOS_BC_PERIODIC 0 /* communication boundary onto the same block: wrap copy */
