@@ -61,8 +61,6 @@ def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto", shape=(
     tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0
     if prec == 0 and (variant == "tma" or (variant == "auto" and tma_ok)):
         return f"stage_tma<{stage}>"
-    if prec == 0 and variant == "roles":
-        return f"stage_roles<{stage}>"
     if prec == 0 and variant in ("auto", "paired"):
         return f"stage_pair<{stage},{ndim}>"
     return f"stage_tiled<{'float' if prec == 0 else 'double'},{stage},{ndim}>"
@@ -201,7 +199,7 @@ def run_ours(args):
     ncell = pr.ncell
     stream = torch.cuda.Stream()
     variant = {"auto": binding.KERNEL_AUTO, "simple": binding.KERNEL_SIMPLE, "tiled": binding.KERNEL_TILED,
-               "paired": binding.KERNEL_PAIRED, "roles": binding.KERNEL_ROLES, "tma": binding.KERNEL_TMA}[args.kernel]
+               "paired": binding.KERNEL_PAIRED, "tma": binding.KERNEL_TMA}[args.kernel]
     vanleer = args.integrator == "vanleer"
     bpc = dict(BYTES_PER_CELL)
     if vanleer:
@@ -334,7 +332,7 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "roles", "tma"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "tma"],
                     help="stage kernel variant (default: the library's own choice)")
     ap.add_argument("--integrator", default="heun", choices=["heun", "vanleer"],
                     help="time integrator (PAPER.md Sec. 3.3); the headline metric is quoted on heun")

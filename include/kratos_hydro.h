@@ -29,6 +29,14 @@
  *  - All work is enqueued on the stream given by kratos_hydro_set_stream (default: the
  *    legacy default stream 0).  Calls documented as "asynchronous" return before the GPU
  *    has finished; all others synchronise that stream before returning.
+ *  - The handle remembers the CUDA device that was current at create; every entry point makes
+ *    that device current for its duration and restores the caller's device before returning.
+ *  - Mixed precision only: the fp32 Riemann solver carries the pressure as the deviation from a
+ *    reference pressure p_ref (reading S14).  p_ref = fp32(min(mean p, 2 min p)) of the
+ *    state last given to kratos_hydro_set_state; it is computed by the first cfl_dt / step / run
+ *    after set_state (one extra read of the state) and then kept until the next set_state, so what
+ *    step(dt) computes depends on the state and on dt only, not on which other calls were made.
+ *    With p_ref > 0 the pressure floor of the primitives is max(1e-30, p_ref 2^-22).
  */
 #ifndef KRATOS_HYDRO_H
 #define KRATOS_HYDRO_H
@@ -69,17 +77,19 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
 #define KRATOS_BC_REFLECT 3  /* q(-i-1/2) = q(i+1/2), normal velocity negated */
 
 /* kernel variants (kratos_hydro_set_kernel) */
-#define KRATOS_KERNEL_AUTO 0   /* x,y active: TMA (mixed, 3D, nx % 32 == 0, ny % 16 == 0), else paired (mixed) or tiled
-                                  (all-fp64); otherwise simple */
+#define KRATOS_KERNEL_AUTO 0   /* x,y active: TMA (mixed, 3D, nx % 32 == 0, ny % 16 == 0), strip (mixed, 2D, even extents),
+                                  else paired (mixed) or tiled (all-fp64); otherwise simple */
 #define KRATOS_KERNEL_SIMPLE 1 /* one thread per cell, stencil from global memory (any axes) */
 #define KRATOS_KERNEL_TILED 2  /* shared-memory tile + halo, z marched in registers, each face once */
 #define KRATOS_KERNEL_PAIRED 3 /* mixed precision only: two cells per thread, packed fp32x2 arithmetic,
                                   halo warps, fp64 flux exchange (x,y active) */
-#define KRATOS_KERNEL_ROLES 4  /* mixed precision, three active axes: the paired scheme split over specialised
-                                  warps (z march + update | x,y Riemann problems | halo ring) */
 #define KRATOS_KERNEL_TMA 5    /* the paired scheme with all global traffic moved by TMA boxes (a producer warp loads
                                   tile, halo and U0 planes onto mbarriers and stores each updated plane): mixed
                                   precision, three active axes, nx % 32 == 0, ny % 16 == 0 */
+
+#define KRATOS_KERNEL_STRIP 6  /* 2D blocks (nz = 1, nx and ny even), mixed precision, Heun: one warp per 28-column strip
+                                  marching along y, x neighbours by warp shuffles, row pairs by per-warp TMA boxes; no
+                                  block barriers */
 
 /* Create a solver for an nx*ny*nz block.  gamma > 1.  bc (host, 6 ints) =
  * {x-lo, x-hi, y-lo, y-hi, z-lo, z-hi}; periodic must be set on both sides of an axis or
@@ -100,7 +110,8 @@ KRATOS_API int kratos_hydro_set_stream(kratos_hydro_t *h, void *cuda_stream);
  * support this block's active axes. */
 KRATOS_API int kratos_hydro_set_kernel(kratos_hydro_t *h, int variant);
 
-/* z-extent of the slab one thread block of the tiled kernel marches through (0 = automatic). */
+/* z-extent of the slab one thread block of the marching 3D kernels works through; for the 2D strip kernel the number
+ * of rows (rounded up to even) one warp marches through (0 = automatic). */
 KRATOS_API int kratos_hydro_set_zchunk(kratos_hydro_t *h, int planes);
 
 /* Copy a state in.  U: 5*nx*ny*nz doubles in the layout above; on_device = 0: host pointer
@@ -116,9 +127,10 @@ KRATOS_API int kratos_hydro_get_state(kratos_hydro_t *h, double *U, int on_devic
  * Synchronises.  KRATOS_ERR_NONFINITE if the result is not finite and positive. */
 KRATOS_API int kratos_hydro_cfl_dt(kratos_hydro_t *h, double cfl, double *dt_out);
 
-/* One full Heun step of length dt (> 0, finite; else KRATOS_ERR_ARG):
- *   U1 = U + dt L(U);  U <- 1/2 U + 1/2 (U1 + dt L(U1))        (PAPER.md:264)
- * Asynchronous. */
+/* One full step of length dt (> 0, finite; else KRATOS_ERR_ARG).  Heun:
+ *   U1 = U + dt L(U);  U <- 1/2 U + 1/2 (U1 + dt L(U1))
+ * van Leer (reading S15): W = prim(U + dt/2 L_1(U)); U <- U + dt L(W).
+ * Asynchronous; a non-finite result is reported by kratos_hydro_status, not here. */
 KRATOS_API int kratos_hydro_step(kratos_hydro_t *h, double dt);
 
 /* nsteps Heun steps with the time step kept on the device (no host round trip per step):
@@ -139,6 +151,12 @@ KRATOS_API int kratos_hydro_totals(kratos_hydro_t *h, double out[5]);
 
 /* Number of times a primitive floor (rho, p >= 1e-30) fired since create.  n: host.  Synchronises. */
 KRATOS_API int kratos_hydro_floor_hits(kratos_hydro_t *h, long long *n);
+
+/* Health of the run so far: KRATOS_OK, or KRATOS_ERR_NONFINITE when a time step of run / run_until came out
+ * non-finite or the state left by the last step / run holds a NaN or an infinite wave speed (the final kernel of
+ * every step reduces the CFL rate of the new state, and maps NaN onto +inf), or KRATOS_ERR_CUDA
+ * when an asynchronous launch failed.  Synchronises.  step() itself is asynchronous and cannot report this. */
+KRATOS_API int kratos_hydro_status(kratos_hydro_t *h);
 
 /* Number of kernel launches this handle has issued since create.  n: host.  No synchronisation. */
 KRATOS_API int kratos_hydro_launch_count(kratos_hydro_t *h, long long *n);

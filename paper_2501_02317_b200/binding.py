@@ -19,7 +19,7 @@ from . import build as _build
 PREC_MIXED, PREC_FP64 = 0, 1
 BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
 INTEGRATOR_HEUN, INTEGRATOR_VANLEER = 0 << 4, 1 << 4   # scheme word bits 4-5
-KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_ROLES, KERNEL_TMA = 0, 1, 2, 3, 4, 5
+KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_TMA, KERNEL_STRIP = 0, 1, 2, 3, 5, 6
 OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
 
 # every symbol include/kratos_hydro.h declares
@@ -27,7 +27,7 @@ SYMBOLS = [
     "kratos_hydro_create", "kratos_hydro_destroy", "kratos_hydro_set_spacing", "kratos_hydro_set_stream",
     "kratos_hydro_set_kernel", "kratos_hydro_set_zchunk", "kratos_hydro_set_state", "kratos_hydro_get_state",
     "kratos_hydro_cfl_dt", "kratos_hydro_step", "kratos_hydro_run", "kratos_hydro_run_until",
-    "kratos_hydro_totals", "kratos_hydro_floor_hits", "kratos_hydro_launch_count",
+    "kratos_hydro_totals", "kratos_hydro_floor_hits", "kratos_hydro_status", "kratos_hydro_launch_count",
     "kratos_hydro_set_profiling", "kratos_hydro_get_timing", "kratos_hydro_last_error", "kratos_hydro_version",
 ]
 
@@ -83,6 +83,8 @@ def load() -> ctypes.CDLL:
     L.kratos_hydro_totals.argtypes = [vp, dp]
     L.kratos_hydro_floor_hits.restype = i
     L.kratos_hydro_floor_hits.argtypes = [vp, llp]
+    L.kratos_hydro_status.restype = i
+    L.kratos_hydro_status.argtypes = [vp]
     L.kratos_hydro_launch_count.restype = i
     L.kratos_hydro_launch_count.argtypes = [vp, llp]
     L.kratos_hydro_set_profiling.restype = i
@@ -224,6 +226,10 @@ class KratosHydro:
         n = ctypes.c_longlong(0)
         _check(self._L.kratos_hydro_floor_hits(self._h, ctypes.byref(n)))
         return n.value
+
+    def status(self):
+        """Raises KratosError (ERR_NONFINITE / ERR_CUDA) if the run so far went wrong; synchronises."""
+        _check(self._L.kratos_hydro_status(self._h))
 
     def launch_count(self):
         n = ctypes.c_longlong(0)

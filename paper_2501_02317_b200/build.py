@@ -3,7 +3,12 @@
     python -m paper_2501_02317_b200.build [--force] [--verbose]
 
 nvcc cross-compiles without a GPU.  The built .so is git-ignored but travels to the GPU box
-with the repository snapshot.
+with the repository snapshot.  The ptxas resource report (registers, spills, shared memory per
+kernel) of the last build is left next to it in ``build_ptxas.log`` (git-ignored too).
+
+Supported option: the environment variable ``KH_NVCC_EXTRA`` holds extra nvcc flags, e.g.
+``KH_NVCC_EXTRA="-DKH_TMA_UNROLL=2 -DKH_TMA_MAIN_REGS=200"`` -- the tuning macros the kernel
+headers define under ``#ifndef``.  The default build uses none.
 """
 from __future__ import annotations
 
@@ -16,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkratos_hydro.so")
 SOURCES = ["kh_api.cu"]
-HEADERS = ["kh_device.cuh", "kh_simple.cuh", "kh_tiled.cuh", "kh_pair.cuh", "kh_role.cuh", "kh_tma.cuh", "kh_vanleer.cuh", "kh_reduce.cuh",
+HEADERS = ["kh_device.cuh", "kh_simple.cuh", "kh_tiled.cuh", "kh_pair.cuh", "kh_tma.cuh", "kh_strip.cuh", "kh_vanleer.cuh", "kh_reduce.cuh",
            os.path.join("..", "..", "include", "kratos_hydro.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -43,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    extra = os.environ.get("KH_NVCC_EXTRA", "").split()  # tuning knobs, e.g. -DKH_TY_F32=16 -DKH_BPS_F32=1
+    extra = os.environ.get("KH_NVCC_EXTRA", "").split()  # supported option, see the module docstring
     cmd = [nvcc_path()] + NVCC_FLAGS + extra + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:

@@ -1,6 +1,9 @@
 // kh_api.cu -- the C-ABI of include/kratos_hydro.h: argument checking, memory, launches.
 // No arithmetic of the method lives here; every step of the path runs in the kernels of
-// kh_simple.cuh / kh_tiled.cuh / kh_reduce.cuh.
+// kh_tma.cuh (3D mixed precision: the bench kernel), kh_strip.cuh (2D mixed precision), kh_pair.cuh (mixed
+// precision, other blocks with active x and y), kh_tiled.cuh (all-fp64), kh_simple.cuh (any axes), kh_vanleer.cuh (van Leer integrator, general
+// blocks) and kh_reduce.cuh (CFL rate, reference pressure, dt bookkeeping, totals); kh_device.cuh holds the
+// shared device functions.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -14,8 +17,8 @@
 #include "kh_simple.cuh"
 #include "kh_tiled.cuh"
 #include "kh_pair.cuh"
-#include "kh_role.cuh"
 #include "kh_tma.cuh"
+#include "kh_strip.cuh"
 #include "kh_vanleer.cuh"
 
 using namespace kh;
@@ -40,7 +43,7 @@ static int fail(int code, const char* fmt, ...)
     } while (0)
 
 enum { SLOT_STAGE1 = 0, SLOT_STAGE2 = 1, SLOT_OTHER = 2 };
-enum { CFL_MAX_BLOCKS = 148 * 8 };
+enum { CFL_MAX_BLOCKS = 148 * 8 };   // p_partial holds 2 * CFL_MAX_BLOCKS doubles: block sums, then block minima
 
 struct kratos_hydro {
     Grid g;
@@ -50,6 +53,7 @@ struct kratos_hydro {
     bool tiled_ok;   // tiled kernel supports this block
     int zchunk;      // 0 = auto
     tma::StageMaps* maps;  // tensor maps of the TMA kernel (host; NULL when the block is not supported)
+    strip::StageMaps* smaps;  // tensor maps of the 2D strip kernel (host; NULL when the block is not supported)
     double* U0;      // current state (device)
     double* U1;      // Heun: predictor state, 5 N fp64.  van Leer: W^{n+1/2}, 5 N float_t primitives (device)
     Ctrl* ctrl;      // device
@@ -59,7 +63,9 @@ struct kratos_hydro {
     double* p_partial;  // per-block pressure sums of the cfl kernel (device)
     int tot_blocks;
     cudaStream_t stream;
+    int device;       // CUDA device the handle lives on (every entry point runs with it current)
     bool rate_valid;  // ctrl->rate_bits holds the rate maximum of U0
+    bool pref_valid;  // ctrl->p_ref was computed from the state last given to set_state
     long long launches;
     // profiling
     bool profiling;
@@ -75,6 +81,18 @@ const char* kratos_hydro_version(void) { return "kratos-hydro-b200 0.1 (sm_100a)
 
 // ---------------------------------------------------------------------------------------
 namespace {
+
+// Makes the handle's device current for the duration of an entry point (a caller may have switched devices
+// since create) and restores the caller's device afterwards.
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(const kratos_hydro* h) : prev(-1), switched(false)
+    {
+        if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->device) switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 struct LaunchTimer {
     kratos_hydro* h;
@@ -123,15 +141,17 @@ int auto_variant(const kratos_hydro* h)
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
     if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
-    return KRATOS_KERNEL_PAIRED;  // fastest measured on B200
+    if (h->smaps && h->smaps->ok) return KRATOS_KERNEL_STRIP;
+    return KRATOS_KERNEL_PAIRED;
 }
 
 int pick_zchunk(const kratos_hydro* h)
 {
+    if (h->zchunk > 0 && h->variant == KRATOS_KERNEL_STRIP) return h->zchunk < h->g.n[1] ? h->zchunk : h->g.n[1];
     if (h->zchunk > 0) return h->zchunk < h->g.n[2] ? h->zchunk : h->g.n[2];
     if (h->variant == KRATOS_KERNEL_TMA) return tma::auto_zchunk(h->g);
-    return (h->variant == KRATOS_KERNEL_PAIRED || h->variant == KRATOS_KERNEL_ROLES) ? pr::auto_zchunk(h->g)
-                                                                                      : tiled_auto_zchunk(h->g);
+    if (h->variant == KRATOS_KERNEL_STRIP) return strip::auto_rows(h->g);
+    return (h->variant == KRATOS_KERNEL_PAIRED) ? pr::auto_zchunk(h->g) : tiled_auto_zchunk(h->g);
 }
 
 template <typename T>
@@ -143,8 +163,8 @@ int launch_stage(kratos_hydro* h, int stage)
     LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
     if (h->variant == KRATOS_KERNEL_TMA) {
         tma::launch_stage(stage, *h->maps, g, h->ctrl, pick_zchunk(h), h->stream);
-    } else if (h->variant == KRATOS_KERNEL_ROLES) {
-        rl::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
+    } else if (h->variant == KRATOS_KERNEL_STRIP) {
+        strip::launch_stage(stage, *h->smaps, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_PAIRED) {
         pr::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_TILED) {
@@ -198,12 +218,17 @@ int launch_cfl_rate(kratos_hydro* h)
         long long blocks = (h->g.N + 255) / 256;
         if (blocks > CFL_MAX_BLOCKS) blocks = CFL_MAX_BLOCKS;
         cfl_rate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl, h->p_partial);
-        finish_cfl_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, h->p_partial, (int)blocks, 1.0 / (double)h->g.N);
-        h->launches++;
+        // the reference pressure is a function of the state given to set_state and of nothing else: calling
+        // cfl_dt() between steps must not change what the following steps compute
+        if (!h->pref_valid) {
+            finish_cfl_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, h->p_partial, (int)blocks, 1.0 / (double)h->g.N);
+            h->launches++;
+        }
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "cfl launch: %s", cudaGetErrorString(e));
     h->rate_valid = true;
+    h->pref_valid = true;
     return KRATOS_OK;
 }
 
@@ -281,10 +306,14 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->integ = integ;
     h->tiled_ok = g.active[0] && g.active[1] && integ == 0;   // the fused stage kernels are the Heun path
     h->maps = nullptr;
+    h->smaps = nullptr;
     h->variant = auto_variant(h);
     h->zchunk = 0;
     h->stream = 0;
+    h->device = 0;
+    cudaGetDevice(&h->device);
     h->rate_valid = false;
+    h->pref_valid = false;
     h->launches = 0;
     h->profiling = false;
     h->ev_next = 0;
@@ -301,7 +330,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         (e = cudaMalloc(&h->ctrl, sizeof(Ctrl))) != cudaSuccess ||
         (e = cudaMalloc(&h->partial, sizeof(dd) * 5 * h->tot_blocks)) != cudaSuccess ||
         (e = cudaMalloc(&h->d_tot, sizeof(double) * 5)) != cudaSuccess ||
-        (e = cudaMalloc(&h->p_partial, sizeof(double) * CFL_MAX_BLOCKS)) != cudaSuccess ||
+        (e = cudaMalloc(&h->p_partial, sizeof(double) * 2 * CFL_MAX_BLOCKS)) != cudaSuccess ||
         (e = cudaMallocHost(&h->h_ctrl, sizeof(Ctrl) + 64)) != cudaSuccess ||
         (e = cudaMemset(h->ctrl, 0, sizeof(Ctrl))) != cudaSuccess ||
         (e = cudaMemset(h->U0, 0, bytes)) != cudaSuccess || (e = cudaMemset(h->U1, 0, bytes1)) != cudaSuccess) {
@@ -312,12 +341,16 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     }
     tiled_configure();
     pr::configure();
-    rl::configure();
     tma::configure();
+    strip::configure();
     if (prec == KRATOS_PREC_MIXED && tma::supported(g)) {
         h->maps = new (std::nothrow) tma::StageMaps;
         if (h->maps && integ == 0) tma::build_maps(h->maps, h->U0, h->U1, g);
         if (h->maps && integ == 1) tma::build_maps_vl(h->maps, h->U0, (const float*)h->U1, g);
+    }
+    if (prec == KRATOS_PREC_MIXED && integ == 0 && strip::supported(g)) {
+        h->smaps = new (std::nothrow) strip::StageMaps;
+        if (h->smaps) strip::build_maps(h->smaps, h->U0, h->U1, g);
     }
     h->variant = auto_variant(h);
     return h;
@@ -326,6 +359,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
 void kratos_hydro_destroy(kratos_hydro_t* h)
 {
     if (!h) return;
+    DeviceGuard dg(h);
     cudaFree(h->U0);
     cudaFree(h->U1);
     cudaFree(h->ctrl);
@@ -334,6 +368,7 @@ void kratos_hydro_destroy(kratos_hydro_t* h)
     cudaFree(h->p_partial);
     if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
     delete h->maps;
+    delete h->smaps;
     for (auto e : h->ev_pool) cudaEventDestroy(e);
     delete h;
 }
@@ -362,14 +397,14 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
     if (variant == KRATOS_KERNEL_AUTO) variant = auto_variant(h);
     if ((variant == KRATOS_KERNEL_TILED || variant == KRATOS_KERNEL_PAIRED) && !h->tiled_ok)
         return fail(KRATOS_ERR_ARG, "tiled and paired kernels need active x and y axes");
-    if ((variant == KRATOS_KERNEL_PAIRED || variant == KRATOS_KERNEL_ROLES) && h->prec != KRATOS_PREC_MIXED)
-        return fail(KRATOS_ERR_ARG, "the paired and role-split kernels are the mixed-precision path");
-    if (variant == KRATOS_KERNEL_ROLES && (!h->tiled_ok || !h->g.active[2]))
-        return fail(KRATOS_ERR_ARG, "the role-split kernel needs three active axes");
+    if (variant == KRATOS_KERNEL_PAIRED && h->prec != KRATOS_PREC_MIXED)
+        return fail(KRATOS_ERR_ARG, "the paired kernel is the mixed-precision path");
     if (variant == KRATOS_KERNEL_TMA && !(h->maps && h->maps->ok))
         return fail(KRATOS_ERR_ARG, "the TMA kernel needs mixed precision, three active axes, nx %% 32 == 0 and ny %% 16 == 0");
+    if (variant == KRATOS_KERNEL_STRIP && !(h->smaps && h->smaps->ok))
+        return fail(KRATOS_ERR_ARG, "the strip kernel needs mixed precision, the Heun integrator and a 2D block (nz = 1) with even nx, ny");
     if (variant != KRATOS_KERNEL_SIMPLE && variant != KRATOS_KERNEL_TILED && variant != KRATOS_KERNEL_PAIRED &&
-        variant != KRATOS_KERNEL_ROLES && variant != KRATOS_KERNEL_TMA)
+        variant != KRATOS_KERNEL_TMA && variant != KRATOS_KERNEL_STRIP)
         return fail(KRATOS_ERR_ARG, "bad variant");
     h->variant = variant;
     return KRATOS_OK;
@@ -386,9 +421,11 @@ int kratos_hydro_set_state(kratos_hydro_t* h, const double* U, int on_device)
 {
     if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
     const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
+    DeviceGuard dg(h);
     CUDA_TRY(cudaMemcpyAsync(h->U0, U, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
     if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
     h->rate_valid = false;
+    h->pref_valid = false;
     return KRATOS_OK;
 }
 
@@ -396,6 +433,7 @@ int kratos_hydro_get_state(kratos_hydro_t* h, double* U, int on_device)
 {
     if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
     const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
+    DeviceGuard dg(h);
     CUDA_TRY(cudaMemcpyAsync(U, h->U0, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
     if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
     return KRATOS_OK;
@@ -405,6 +443,7 @@ int kratos_hydro_cfl_dt(kratos_hydro_t* h, double cfl, double* dt_out)
 {
     if (!h || !dt_out) return fail(KRATOS_ERR_ARG, "NULL argument");
     if (!(cfl > 0.0) || !std::isfinite(cfl)) return fail(KRATOS_ERR_ARG, "cfl must be > 0");
+    DeviceGuard dg(h);
     int rc;
     if ((rc = launch_cfl_rate(h))) return rc;
     if ((rc = read_ctrl(h))) return rc;
@@ -420,12 +459,15 @@ int kratos_hydro_step(kratos_hydro_t* h, double dt)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(KRATOS_ERR_ARG, "dt must be > 0 and finite");
+    DeviceGuard dg(h);
+    int rc;
+    // first step after set_state: the reference pressure of the mixed-precision kernels comes from this state
+    if (!h->pref_valid && h->prec == KRATOS_PREC_MIXED && (rc = launch_cfl_rate(h))) return rc;
     {
         LaunchTimer lt(h, SLOT_OTHER);
         set_dt_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, dt);
     }
-    int rc = launch_both_stages(h);
-    if (rc) return rc;
+    if ((rc = launch_both_stages(h))) return rc;
     h->rate_valid = true;  // stage 2 left the rate maximum of the new state in ctrl
     return KRATOS_OK;
 }
@@ -435,14 +477,18 @@ static int run_impl(kratos_hydro_t* h, double cfl, double t_end, int max_steps, 
     if (!h || !t_inout) return fail(KRATOS_ERR_ARG, "NULL argument");
     if (!(cfl > 0.0) || !std::isfinite(cfl) || max_steps < 0) return fail(KRATOS_ERR_ARG, "bad cfl / step count");
     if (!std::isfinite(*t_inout) || !std::isfinite(t_end)) return fail(KRATOS_ERR_ARG, "non-finite time");
+    DeviceGuard dg(h);
     int rc;
     {
         LaunchTimer lt(h, SLOT_OTHER);
         configure_run_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, cfl, t_end > 0.0 ? t_end : 0.0, *t_inout);
     }
-    if (!h->rate_valid && (rc = launch_cfl_rate(h))) return rc;
+    if ((!h->rate_valid || !h->pref_valid) && (rc = launch_cfl_rate(h))) return rc;
     int done = 0;
-    const int batch = (t_end > 0.0) ? 64 : max_steps;
+    // run_until: steps are enqueued in batches and the host looks at t between batches.  The batch shrinks to
+    // the number of steps the last dt predicts are left (+1), so that hardly any zero-length step is enqueued
+    // after t has reached t_end.
+    int batch = (t_end > 0.0) ? 8 : max_steps;
     while (done < max_steps) {
         const int nb = (max_steps - done < batch) ? max_steps - done : batch;
         for (int s = 0; s < nb; s++) {
@@ -455,7 +501,11 @@ static int run_impl(kratos_hydro_t* h, double cfl, double t_end, int max_steps, 
         done += nb;
         if ((rc = read_ctrl(h))) return rc;
         if (h->h_ctrl->nonfinite) break;
-        if (t_end > 0.0 && h->h_ctrl->t >= t_end) break;
+        if (t_end > 0.0) {
+            if (h->h_ctrl->t >= t_end) break;
+            const double left = (t_end - h->h_ctrl->t) / (h->h_ctrl->dt > 0.0 ? h->h_ctrl->dt : t_end);
+            batch = left > 63.0 ? 64 : (int)left + 1;
+        }
     }
     if (done == 0 && (rc = read_ctrl(h))) return rc;
     *t_inout = h->h_ctrl->t;
@@ -481,6 +531,7 @@ int kratos_hydro_run_until(kratos_hydro_t* h, double cfl, double t_end, int max_
 int kratos_hydro_totals(kratos_hydro_t* h, double out[5])
 {
     if (!h || !out) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
     {
         LaunchTimer lt(h, SLOT_OTHER);
         totals_kernel<<<dim3(h->tot_blocks, 5), 256, 0, h->stream>>>(h->U0, h->g.N, h->partial);
@@ -500,9 +551,28 @@ int kratos_hydro_totals(kratos_hydro_t* h, double out[5])
 int kratos_hydro_floor_hits(kratos_hydro_t* h, long long* n)
 {
     if (!h || !n) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
     int rc = read_ctrl(h);
     if (rc) return rc;
     *n = (long long)h->h_ctrl->floor_hits;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_status(kratos_hydro_t* h)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    DeviceGuard dg(h);
+    int rc = read_ctrl(h);
+    if (rc) return rc;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "status: %s", cudaGetErrorString(e));
+    if (h->h_ctrl->nonfinite) return fail(KRATOS_ERR_NONFINITE, "a time step came out non-finite (t = %g)", h->h_ctrl->t);
+    if (h->rate_valid) {
+        // the final kernel of every step reduces the CFL rate of the new state and maps NaN onto +inf
+        double rate;
+        memcpy(&rate, &h->h_ctrl->rate_bits, sizeof(double));
+        if (!(rate < HUGE_VAL)) return fail(KRATOS_ERR_NONFINITE, "non-finite state (CFL rate %g, t = %g)", rate, h->h_ctrl->t);
+    }
     return KRATOS_OK;
 }
 
@@ -516,6 +586,7 @@ int kratos_hydro_launch_count(kratos_hydro_t* h, long long* n)
 int kratos_hydro_set_profiling(kratos_hydro_t* h, int enable)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    DeviceGuard dg(h);
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     h->ev_used.clear();
     h->ev_next = 0;
@@ -527,6 +598,7 @@ int kratos_hydro_set_profiling(kratos_hydro_t* h, int enable)
 int kratos_hydro_get_timing(kratos_hydro_t* h, double ms[3], long long launches[3])
 {
     if (!h || !ms || !launches) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     collect_timing(h);
     for (int s = 0; s < 3; s++) { ms[s] = h->prof_ms[s]; launches[s] = h->prof_n[s]; }

@@ -150,6 +150,10 @@ __device__ __forceinline__ void face_flux2(const f2 qL[5], const f2 qR[5], const
 // rounded so that every copy (main warps, halo warps, neighbouring blocks) returns the same bits;
 // 1/rho by MUFU.RCP64H + one Newton step (2^-40, far below the fp32 rounding of the result).
 // Boundary rules act on the normal velocities.  Returns the floor activations (S6).
+// With a reference pressure the floor is max(1e-30, pref 2^-22): two fp32 ulps of pref, so that the stored
+// deviation p - pref never rounds to -pref and the pressure rebuilt by the Riemann solver stays > 0 (the
+// limited face states lie between the cell values, Eq. 3).  pref <= 2 p_min when it is set (kh_reduce.cuh),
+// so this floor is 5e-7 of the lowest pressure the block held then.
 __device__ __forceinline__ int recover(double rho, double mx, double my, double mz, double e, double gm1, double pref,
                                        int rx, int ry, int rz, float W[5])
 {
@@ -162,8 +166,9 @@ __device__ __forceinline__ int recover(double rho, double mx, double my, double 
     // (m.m)/rho with m.m formed first: it does not wait for the reciprocal, which shortens the dependent chain
     const double m2 = __dmul_rn(__fma_rn(mz, mz, __fma_rn(my, my, __dmul_rn(mx, mx))), ir);
     double p = __dmul_rn(gm1, __fma_rn(-0.5, m2, e));
-    const bool lo_p = p < KH_P_FLOOR;
-    p = lo_p ? KH_P_FLOOR : p;
+    const double pfl = fmax(KH_P_FLOOR, __dmul_rn(pref, 0x1p-22));
+    const bool lo_p = p < pfl;
+    p = lo_p ? pfl : p;
     if (rx | ry | rz) {
         vx = apply_vn_rule(vx, rx);
         vy = apply_vn_rule(vy, ry);

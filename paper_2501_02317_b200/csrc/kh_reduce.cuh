@@ -6,13 +6,14 @@ namespace kh {
 
 // CFL rate maximum of the stored state, fp64 in every precision mode (S1, S7).
 // Grid-stride, warp-shuffle + one atomicMax per block.  Also leaves each block's pressure sum in
-// p_partial[blockIdx.x] (fixed reduction order => run-to-run reproducible reference pressure).
+// p_partial[blockIdx.x] and its pressure minimum in p_partial[gridDim.x + blockIdx.x] (fixed reduction
+// order => run-to-run reproducible reference pressure).
 __global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict__ U, Grid g, Ctrl* ctrl,
                                                        double* p_partial)
 {
     __shared__ double red[32];
-    __shared__ double psum[8];
-    double rate = 0.0, ps = 0.0;
+    __shared__ double psum[8], pmin[8];
+    double rate = 0.0, ps = 0.0, pm = __longlong_as_double(0x7ff0000000000000LL);
     const CflConst<double> cc(g);
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < g.N;
          c += (long long)gridDim.x * blockDim.x) {
@@ -22,24 +23,32 @@ __global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict_
         if (!(r == r)) r = __longlong_as_double(0x7ff0000000000000LL);
         rate = fmax(rate, r);
         ps += p;
+        pm = fmin(pm, p);
     }
-    for (int o = 16; o > 0; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
-    if ((threadIdx.x & 31) == 0) psum[threadIdx.x >> 5] = ps;
+    for (int o = 16; o > 0; o >>= 1) {
+        ps += __shfl_xor_sync(0xffffffffu, ps, o);
+        pm = fmin(pm, __shfl_xor_sync(0xffffffffu, pm, o));
+    }
+    if ((threadIdx.x & 31) == 0) { psum[threadIdx.x >> 5] = ps; pmin[threadIdx.x >> 5] = pm; }
     block_atomic_max_nonneg(rate, &ctrl->rate_bits, red);  // contains a __syncthreads()
     if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int w = 0; w < 8; w++) t += psum[w];
+        double t = 0.0, m = pmin[0];
+        for (int w = 0; w < 8; w++) { t += psum[w]; m = fmin(m, pmin[w]); }
         p_partial[blockIdx.x] = t;
+        p_partial[gridDim.x + blockIdx.x] = m;
     }
 }
 
-// Reference pressure of the mixed-precision momentum flux: the mean pressure, rounded to fp32 so that
-// the fp64 primitive recovery and the fp32 Riemann solver use the very same number.
+// Reference pressure of the mixed-precision momentum flux (reading S14): min(mean pressure,
+// 2 x minimum pressure), rounded to fp32 so that the fp64 primitive recovery and the fp32 Riemann solver
+// use the very same number.  The stored deviation p - p_ref of a cell then has the absolute error
+// ulp_fp32(|p - p_ref|) <= ulp_fp32(p) wherever p >= p_min: never worse than plain fp32 pressure, and far
+// better where the pressure is nearly uniform (the mean is then below 2 p_min and is the reference).
 __global__ void finish_cfl_kernel(Ctrl* ctrl, const double* p_partial, int nblocks, double inv_n)
 {
-    double t = 0.0;
-    for (int b = 0; b < nblocks; b++) t += p_partial[b];
-    const float m = (float)(t * inv_n);
+    double t = 0.0, pm = p_partial[nblocks];
+    for (int b = 0; b < nblocks; b++) { t += p_partial[b]; pm = fmin(pm, p_partial[nblocks + b]); }
+    const float m = (float)fmin(t * inv_n, 2.0 * pm);
     ctrl->p_ref = (m == m && m > 0.0f && m < 3.0e38f) ? (double)m : 0.0;
 }
 

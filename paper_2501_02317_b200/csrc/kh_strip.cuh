@@ -1,0 +1,354 @@
+// kh_strip.cuh -- KRATOS_KERNEL_STRIP: the fused stage kernel of 2D blocks (x and y active, nz == 1) in mixed
+// precision (float_t = fp32, float2_t = fp64): one warp = one independent pipeline.
+//
+// A warp owns a strip of SW = 28 columns and marches along y through a slab of rows, two rows per trip:
+//   * lane l holds column x0 - 2 + l of the strip's 32-column window; the two outer lanes on either side are the
+//     2-cell halo of the PLM stencil and are recomputed by the neighbouring strip (28 of 32 lanes produce output),
+//     so every x neighbour of a cell lives in the neighbouring LANE: slopes, left states and fluxes cross the strip
+//     by warp shuffles, and a warp never waits for another warp -- no block barrier anywhere in the kernel;
+//   * a thread holds the row pair (2p, 2p+1) packed as f32x2, like the 3D kernels hold (2w, 2w+1): the slopes of
+//     Eq. 3 and the HLLC solver of Eq. 4-5 run on packed FADD2 / FMUL2 / FFMA2, the x faces and the y faces of the pair
+//     in lock step (tma::hllc2n<2>).  The y face between the two rows is internal to the thread; the face below the
+//     pair was solved one trip earlier and the one above it is solved one trip later, so the march carries the
+//     limited state of the last row and the fp64 flux sum of the pair, and the pair is updated one trip after it was
+//     solved: the y direction lives in registers, as z does in the 3D kernels;
+//   * global -> shared traffic is one TMA box (32 x 2 x 5 doubles) per row pair and warp, prefetched three pairs ahead
+//     into a ring of NRING slots, completing on the warp's own mbarriers; at the domain edge two extra 2-column boxes
+//     bring the ghost columns from where the boundary rule of Sec. 3.1.1 takes them (periodic wrap,
+//     clamp, mirror), and ghost rows are a choice of box coordinates, exactly as in kh_tma.cuh;
+//   * the update is fp64: raw state from the ring + flux sums, Heun average with U0 (plain
+//     coalesced loads issued one trip ahead), coalesced 8-byte stores; stage 2 reduces the CFL rate of the new state
+//     (PAPER.md:173).
+// Warps are independent, so their load, convert, solve and update phases interleave on the SM by themselves; 12 warps
+// per SM (three blocks of four warps).
+//
+// Bit-identical fluxes across strip and slab seams: both copies of a shared face run the same explicitly rounded
+// operations (kh_pair.cuh) on the same inputs, so the fp64 contributions cancel exactly.
+#pragma once
+#include "kh_tma.cuh"
+
+namespace kh {
+namespace strip {
+
+using pr::f2;
+using pr::mk;
+using pr::plm;
+using pr::recover;
+using pr::Gas;
+using tma::HaloSide;
+using tma::halo_side;
+
+constexpr int SW = 28;        // columns of output per warp (lanes 2..29 of the 32-lane window)
+constexpr int NRING = 5;      // row pairs in flight per warp: p-1 (update), p, p+1 (converted ahead), p+2, p+3 (arriving)
+constexpr int WARPS = 4;      // warps per block (independent of each other)
+constexpr int BLOCKS_PER_SM = 3;
+constexpr unsigned BOX_BYTES = 5 * 2 * 32 * 8;   // 2560
+constexpr unsigned HBOX_BYTES = 5 * 2 * 2 * 8;   // 160
+
+struct WarpSmem {
+    alignas(128) double raw[NRING][5][2][32];    // TMA box of a row pair: [field][row][column]
+    alignas(128) double hx[NRING][2][32];        // ghost-column boxes [side][5 fields x 2 rows x 2 columns], padded to 256 B
+    unsigned long long full[NRING];
+};
+
+struct Maps {
+    CUtensorMap in_own, in_cols;   // stage input: 32 x 2 x 5 box, 2 x 2 x 5 box
+};
+
+__device__ __forceinline__ void tma_load3(void* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
+            "r"(tma::smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(tma::smem_u32(bar))
+        : "memory");
+}
+
+__device__ __forceinline__ f2 shfl_up2(f2 v)
+{
+    return mk(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1));
+}
+__device__ __forceinline__ f2 shfl_down2(f2 v)
+{
+    return mk(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1));
+}
+
+// One Heun stage of a 2D block.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin +
+// dt L(Uin)) (Uout aliases U0) and the CFL rate maximum of Uout.
+// rows_per_slab is even; a warp handles strip (id % nstrips), slab (id / nstrips).
+template <int STAGE>
+__global__ void __launch_bounds__(WARPS * 32, BLOCKS_PER_SM)
+stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, Grid g, Ctrl* ctrl, int rows_per_slab,
+            int nstrips, int nwork)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpSmem& sm = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+
+    const double dt = ctrl->dt;
+    if (!(dt > 0.0)) return;  // a step clipped to zero length (run_until past t_end) does nothing
+    const int work = blockIdx.x * WARPS + warp;
+    if (work >= nwork) return;   // (whole warps: no block-wide synchronisation exists in this kernel)
+    const double pref_d = ctrl->p_ref;
+    const int nx = g.n[0], ny = g.n[1];
+    const long long N = g.N;
+    const int s = work % nstrips, slab = work / nstrips;
+    const int x0 = s * SW;                         // first output column
+    const int c = x0 - 2 + lane;                   // this lane's column
+    const int npair = ny / 2;
+    const int pbeg = slab * (rows_per_slab / 2);
+    const int pend = min(pbeg + rows_per_slab / 2, npair);   // pairs [pbeg, pend)
+    const double gm1 = g.gamma - 1.0;
+    Gas gas;
+    gas.gamma = (float)g.gamma;
+    gas.g1 = (float)((g.gamma + 1.0) / (2.0 * g.gamma));
+    gas.igm1 = (float)(1.0 / (g.gamma - 1.0));
+    gas.pref = (float)pref_d;
+
+    // ---- where this lane's column comes from (Sec. 3.1.1 in x) ----
+    // interior column: the strip's own box.  Ghost column (c in {-2,-1} or {nx, nx+1}): one of the two ghost boxes.
+    const HaloSide xlo = halo_side(-2, nx, g.bc[0], g.bc[1]);
+    const HaloSide xhi = halo_side(nx, nx, g.bc[0], g.bc[1]);
+    const bool ghost_lo = c < 0, ghost_hi = c >= nx && c < nx + 2;
+    const bool need_lo = x0 - 2 < 0, need_hi = x0 - 2 + 32 > nx;      // warp-uniform: this strip touches a domain edge
+    const int rx = ghost_lo ? xlo.rule : (ghost_hi ? xhi.rule : VN_KEEP);
+    const int hx_idx = ghost_lo ? ((c == -2) ? xlo.idx0 : xlo.idx1) : ((c == nx) ? xhi.idx0 : xhi.idx1);
+    const bool owner = lane >= 2 && lane < 2 + SW && c < nx;          // this lane's cells are written by this warp
+    // element offsets of this lane inside a ring slot: own box [field][row][32], ghost box [side][field][row][2]
+    const double* const own_base = &sm.raw[0][0][0][lane];
+    const double* const hx_base = &sm.hx[0][ghost_hi ? 1 : 0][hx_idx];
+    const bool from_ghost_box = ghost_lo || ghost_hi;
+
+    if (lane == 0) {
+        for (int q = 0; q < NRING; q++) mbar_init(&sm.full[q], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    // pair q (rows 2q, 2q+1; q in [-1, npair]) -> the box rows that hold it (Sec. 3.1.1 in y)
+    auto issue = [&](int q) {   // lane 0
+        const HaloSide ys = halo_side(2 * q, ny, g.bc[2], g.bc[3]);
+        const int slot = (q + NRING) % NRING;
+        unsigned long long* bar = &sm.full[slot];
+        tma::mbar_expect_tx(bar, BOX_BYTES + (need_lo ? HBOX_BYTES : 0u) + (need_hi ? HBOX_BYTES : 0u));
+        tma_load3(&sm.raw[slot][0][0][0], &maps.in_own, x0 - 2, ys.start, 0, bar);
+        if (need_lo) tma_load3(&sm.hx[slot][0][0], &maps.in_cols, xlo.start, ys.start, 0, bar);
+        if (need_hi) tma_load3(&sm.hx[slot][1][0], &maps.in_cols, xhi.start, ys.start, 0, bar);
+    };
+    // The ring is indexed by (q mod NRING); each slot's mbarrier flips once per use.
+    unsigned phase_bits = 0u;   // bit `slot`: parity to wait for next
+    int hits = 0;
+    auto convert = [&](int q, f2 W[5], bool count) {
+        const HaloSide ys = halo_side(2 * q, ny, g.bc[2], g.bc[3]);
+        const int slot = (q + NRING) % NRING;
+        tma::mbar_wait_parity(&sm.full[slot], (phase_bits >> slot) & 1u);
+        phase_bits ^= 1u << slot;
+        double ua[5], ub[5];
+        if (from_ghost_box) {
+            const double* b = hx_base + slot * (2 * 32);
+#pragma unroll
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 4 + ys.idx0 * 2]; ub[f] = b[f * 4 + ys.idx1 * 2]; }
+        } else {
+            const double* b = own_base + slot * (5 * 2 * 32);
+#pragma unroll
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 64 + ys.idx0 * 32]; ub[f] = b[f * 64 + ys.idx1 * 32]; }
+        }
+        float Wa[5], Wb[5];
+        const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, ys.rule, VN_KEEP, Wa);
+        const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, ys.rule, VN_KEEP, Wb);
+        if (count && owner) hits += ha + hb;
+#pragma unroll
+        for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
+    };
+
+    // ---- prologue: pairs pbeg-1 .. pbeg+2 in flight, W(pbeg-1) and W(pbeg) converted ----
+    if (lane == 0)
+        for (int q = pbeg - 1; q <= min(pbeg + 2, pend); q++) issue(q);
+    f2 Wm[5], W0[5], Wp[5];
+    convert(pbeg - 1, Wm, false);
+    convert(pbeg, W0, true);
+    float QLc[5];                 // left state of the y face below row 2p (limited state of row 2p-1 at its upper face)
+    double2 dUprev[5];            // flux sums of pair p-1: row 2p-2 complete, row 2p-1 lacks the face above it
+#pragma unroll
+    for (int f = 0; f < 5; f++) {
+        f2 qL, qR;
+        plm(mk(Wm[f].x, Wm[f].x), Wm[f], mk(Wm[f].y, W0[f].x), qL, qR);   // row 2pbeg-1 from rows 2pbeg-2, 2pbeg-1, 2pbeg
+        QLc[f] = qL.y;
+        dUprev[f] = make_double2(0.0, 0.0);
+    }
+    const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1];
+    const CflConst<float> cc(g);
+    f2 rate = mk(0.0f, 0.0f);
+    const long long col_off = (long long)(owner ? c : 0);
+
+    // trip p solves the faces of pair p and completes the update of pair p-1; the last trip (p == pend) only completes
+#pragma unroll 1
+    for (int p = pbeg; p <= pend; p++) {
+        if (lane == 0 && p + 3 <= pend) issue(p + 3);    // into the slot pair p-2 left after its update in trip p-1
+        const bool upd = (p > pbeg) && owner;
+        const long long cell_prev = (long long)(2 * (p - 1)) * nx + col_off;
+        if (p + 1 <= pend) convert(p + 1, Wp, p + 1 < pend);
+        // ---- slopes (Eq. 3) and the two face pairs of pair p ----
+        f2 L[2][5], R[2][5], Fn[2][5];
+        {
+            f2 qLx[5], qRx[5], qLy[5], qRy[5];
+#pragma unroll
+            for (int f = 0; f < 5; f++) {
+                const f2 xm = shfl_up2(W0[f]), xp = shfl_down2(W0[f]);
+                plm(xm, W0[f], xp, qLx[f], qRx[f]);
+                plm(mk(Wm[f].y, W0[f].x), W0[f], mk(W0[f].y, Wp[f].x), qLy[f], qRy[f]);
+            }
+            f2 t[5];
+#pragma unroll
+            for (int f = 0; f < 5; f++) t[f] = shfl_up2(qLx[f]);           // left state of the face at c - 1/2
+            tma::to_normal<0>(t, L[0]);
+            tma::to_normal<0>(qRx, R[0]);
+#pragma unroll
+            for (int f = 0; f < 5; f++) { t[f] = mk(QLc[f], qLy[f].x); QLc[f] = qLy[f].y; }   // faces 2p-1/2, 2p+1/2
+            tma::to_normal<1>(t, L[1]);
+            tma::to_normal<1>(qRy, R[1]);
+        }
+        tma::hllc2n<2>(L, R, gas, Fn);
+        // U0 of pair p-1 for the Heun average: issued here, where the registers of the solver are free again; the other
+        // warps of the SM cover its latency
+        double2 v0[5];
+        if (STAGE == 2 && upd) {
+#pragma unroll
+            for (int f = 0; f < 5; f++) v0[f] = make_double2(U0[f * N + cell_prev], U0[f * N + cell_prev + nx]);
+        }
+        double2 dU[5];
+        {
+            f2 Fx[5], Fy[5];
+            tma::from_normal<0>(Fn[0], Fx);
+            tma::from_normal<1>(Fn[1], Fy);
+#pragma unroll
+            for (int f = 0; f < 5; f++) {
+                const f2 fxh = shfl_down2(Fx[f]);                          // flux through the face at c + 1/2
+                const double flo = (double)Fy[f].x, fin = (double)Fy[f].y;
+                // pair p: x faces of both rows, the y faces 2p-1/2 (+, row 2p) and 2p+1/2 (-, row 2p; +, row 2p+1)
+                dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin),
+                                   __dmul_rn(dtdx, __dadd_rn((double)Fx[f].x, -(double)fxh.x)));
+                dU[f].y = __fma_rn(dtdy, fin, __dmul_rn(dtdx, __dadd_rn((double)Fx[f].y, -(double)fxh.y)));
+                // pair p-1: its upper face is this pair's lower face
+                dUprev[f].y = __fma_rn(-dtdy, flo, dUprev[f].y);
+            }
+        }
+        // ---- fp64 update of pair p-1, in global memory order ----
+        if (upd) {
+            const int slot = (p - 1 + NRING) % NRING;
+            const double* b = own_base + slot * (5 * 2 * 32);
+            double ua[5], ub[5];
+#pragma unroll
+            for (int f = 0; f < 5; f++) {
+                double xa = __dadd_rn(b[f * 64], dUprev[f].x);
+                double xb = __dadd_rn(b[f * 64 + 32], dUprev[f].y);
+                if (STAGE == 2) {
+                    xa = __fma_rn(0.5, v0[f].x, __dmul_rn(0.5, xa));
+                    xb = __fma_rn(0.5, v0[f].y, __dmul_rn(0.5, xb));
+                }
+                ua[f] = xa;
+                ub[f] = xb;
+                Uout[f * N + cell_prev] = xa;
+                Uout[f * N + cell_prev + nx] = xb;
+            }
+            if (STAGE == 2) {   // CFL rate of the new state (readings S1/S7), both rows at once
+                using namespace pr;
+                const float rfl = (float)KH_RHO_FLOOR, pfl = (float)KH_P_FLOOR;
+                f2 r = mk((float)ua[0], (float)ub[0]);
+                r = mk(r.x < rfl ? rfl : r.x, r.y < rfl ? rfl : r.y);  // comparisons, not fmax: a NaN must survive
+                const f2 ir = rcp2(r);
+                const f2 vx = mul2(mk((float)ua[1], (float)ub[1]), ir);
+                const f2 vy = mul2(mk((float)ua[2], (float)ub[2]), ir);
+                const f2 vz = mul2(mk((float)ua[3], (float)ub[3]), ir);
+                const f2 v2 = fma2(vz, vz, fma2(vy, vy, mul2(vx, vx)));
+                f2 pp = mul2(bc(cc.gm1), fma2(mul2(bc(-0.5f), r), v2, mk((float)ua[4], (float)ub[4])));
+                pp = mk(pp.x < pfl ? pfl : pp.x, pp.y < pfl ? pfl : pp.y);
+                const f2 gp = mul2(bc(cc.gamma), pp);
+                const f2 cs = mul2(gp, rsqrt2(mul2(gp, r)));
+                f2 rt = mul2(add2(mk(fabsf(vx.x), fabsf(vx.y)), cs), bc(cc.idx));
+                rt = fma2(add2(mk(fabsf(vy.x), fabsf(vy.y)), cs), bc(cc.idy), rt);
+                if (!(rt.x == rt.x)) rt.x = __int_as_float(0x7f800000);
+                if (!(rt.y == rt.y)) rt.y = __int_as_float(0x7f800000);
+                rate = mk(fmaxf(rate.x, rt.x), fmaxf(rate.y, rt.y));
+            }
+        }
+        __syncwarp();   // every lane has read pair p-1 from the ring before lane 0 refills that slot in the next trip
+#pragma unroll
+        for (int f = 0; f < 5; f++) { Wm[f] = W0[f]; W0[f] = Wp[f]; dUprev[f] = dU[f]; }
+    }
+
+    if (hits) atomicAdd(&ctrl->floor_hits, (unsigned long long)hits);
+    if (STAGE == 2) {
+        float r = fmaxf(rate.x, rate.y);
+        for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
+        if (lane == 0 && r > 0.0f) atomicMax(&ctrl->rate_bits, (unsigned long long)__double_as_longlong((double)r));
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+inline bool supported(const Grid& g)
+{
+    return g.active[0] && g.active[1] && !g.active[2] && g.n[0] % 2 == 0 && g.n[1] % 2 == 0 && g.n[0] >= 4 && g.n[1] >= 4;
+}
+
+// Tensor map over the 2D state U[5][ny][nx] (fp64, x fastest) with a box of bx x 2 x 5.
+inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx)
+{
+    tma::EncodeTiledFn fn = tma::encode_tiled_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], 5};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.n[0] * 8, (cuuint64_t)g.N * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)bx, 2, 5};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+struct StageMaps {
+    Maps s1, s2;   // stage 1 reads A, stage 2 reads B
+    bool ok;
+};
+
+inline void build_maps(StageMaps* sm, const double* A, const double* B, const Grid& g)
+{
+    sm->ok = false;
+    if (!supported(g)) return;
+    if (!make_map(&sm->s1.in_own, A, g, 32) || !make_map(&sm->s1.in_cols, A, g, 2) ||
+        !make_map(&sm->s2.in_own, B, g, 32) || !make_map(&sm->s2.in_cols, B, g, 2))
+        return;
+    sm->ok = true;
+}
+
+inline int auto_rows(const Grid& g)
+{
+    // >= ~4 waves of warps over 148 SMs x 12 warps; slabs of >= 16 rows (every slab converts two extra pairs)
+    const long long nstrips = (g.n[0] + SW - 1) / SW;
+    int rows = g.n[1];
+    while (rows > 16 && nstrips * ((g.n[1] + rows - 1) / rows) < 148LL * WARPS * BLOCKS_PER_SM * 4) rows = ((rows / 2) + 1) & ~1;
+    return rows;
+}
+
+inline void configure()
+{
+    cudaFuncSetAttribute(stage_strip<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem)));
+    cudaFuncSetAttribute(stage_strip<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem)));
+    cudaFuncSetAttribute(stage_strip<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_strip<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
+inline void launch_stage(int stage, const StageMaps& sm, const double* U0, double* Uout, const Grid& g, Ctrl* ctrl, int rows,
+                         cudaStream_t stream)
+{
+    rows = (rows + 1) & ~1;
+    const int nstrips = (g.n[0] + SW - 1) / SW;
+    const int nslabs = (g.n[1] + rows - 1) / rows;
+    const int nwork = nstrips * nslabs;
+    const unsigned blocks = (unsigned)((nwork + WARPS - 1) / WARPS);
+    const size_t smem = WARPS * sizeof(WarpSmem);
+    if (stage == 1) stage_strip<1><<<blocks, WARPS * 32, smem, stream>>>(sm.s1, U0, Uout, g, ctrl, rows, nstrips, nwork);
+    else            stage_strip<2><<<blocks, WARPS * 32, smem, stream>>>(sm.s2, U0, Uout, g, ctrl, rows, nstrips, nwork);
+}
+
+}  // namespace strip
+}  // namespace kh

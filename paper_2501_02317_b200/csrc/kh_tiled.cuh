@@ -94,8 +94,9 @@ __device__ __forceinline__ int raw_to_prim(const double u[5], double gm1, double
     double vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
     const double ekin = 0.5 * (u[1] * vx + u[2] * vy + u[3] * vz);
     double p = gm1 * (u[4] - ekin);
-    const bool lo_p = p < KH_P_FLOOR;
-    p = lo_p ? KH_P_FLOOR : p;
+    const double pfl = fmax(KH_P_FLOOR, pref * 0x1p-22);   // see pr::recover (kh_pair.cuh)
+    const bool lo_p = p < pfl;
+    p = lo_p ? pfl : p;
     if (rx | ry | rz) {
         vx = apply_vn_rule(vx, rx);
         vy = apply_vn_rule(vy, ry);

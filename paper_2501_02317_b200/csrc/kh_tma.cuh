@@ -146,26 +146,11 @@ __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commi
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-#ifdef KH_TMA_TIMING   // working instrumentation: cycles spent computing / waiting at the block barrier, per warp
-struct BarTimer { long long t_last, work[2], wait[2], seg[8], t_seg; int n; unsigned addr; };
-// cycles since the previous probe (or barrier) of this warp, accumulated per segment of the main loop
-#define KH_PROBE(i) { long long t_; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t_)::"memory"); bt.seg[i] += t_ - bt.t_seg; bt.t_seg = t_; }
-__device__ __forceinline__ void block_bar_t(BarTimer& bt)
-{
-    long long t0, t1;
-    unsigned x;
-    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t0)::"memory");
-    asm volatile("bar.sync 0;" ::: "memory");
-    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(x) : "r"(bt.addr) : "memory");  // blocks until the barrier opens
-    if (x == 0xdeadbeefu) bt.n += 1000;                                                      // (in-order issue: consumes x)
-    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1)::"memory");
-    bt.work[bt.n & 1] += t0 - bt.t_last; bt.wait[bt.n & 1] += t1 - t0; bt.t_last = t1; bt.t_seg = t1; bt.n++;
-}
-#define block_bar() block_bar_t(bt)
-#else
-#define KH_PROBE(i)
 __device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "memory"); }
-#endif
+
+// Stored pressure deviation of a float_t primitive (van Leer corrector): p - pref with the same two-ulp floor as
+// pr::recover, so that the pressure rebuilt by the Riemann solver stays > 0.
+__device__ __forceinline__ float pdev(float p, float pref_f) { return __fadd_rn(fmaxf(p, pref_f * 0x1p-22f), -pref_f); }
 
 // Where the two halo cells beyond one side of the tile come from (Sec. 3.1.1): first source coordinate of the
 // 2-wide box, the position inside the box of each of the two cells, and the normal-velocity rule.
@@ -351,9 +336,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
     int hits = 0;
     f2 rate = mk(0.0f, 0.0f);
-#ifdef KH_TMA_TIMING
-    BarTimer bt; bt.t_last = clock64(); bt.work[0] = bt.work[1] = bt.wait[0] = bt.wait[1] = 0; bt.n = 0; for (int i = 0; i < 8; i++) bt.seg[i] = 0; bt.t_seg = bt.t_last; bt.addr = smem_u32(&sm.red[0]);
-#endif
 
     if (warp < PRP) {
         // ================================ main warps: cells (i, ja), (i, ja+1) ========================
@@ -385,7 +367,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 const float pref_f = (float)pref_d;
 #pragma unroll
                 for (int f = 0; f < 5; f++) W[f] = mk(sf[f * RAWF], sf[f * RAWF + PTX]);
-                W[1] = mk(__fadd_rn(W[1].x, -pref_f), __fadd_rn(W[1].y, -pref_f));
+                W[1] = mk(pdev(W[1].x, pref_f), pdev(W[1].y, pref_f));
                 W[4] = mk(apply_vn_rule(W[4].x, rz), apply_vn_rule(W[4].y, rz));
                 return;
             }
@@ -458,13 +440,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     to_normal<1>(qL, L[2]);
                     to_normal<1>(QRy, R[2]);
                 }
-                KH_PROBE(0)
                 hllc2n<3>(L, R, gas, Fn);
-                KH_PROBE(1)
                 // plane k+3 (Sec. 3.1): converted here, where the registers of the Riemann solver are free again; its
                 // fp64 chain overlaps the flux accumulation below and phase B(k+1) starts with W(k+3) at hand
                 convert(k + 3, s_conv, par_conv, Wn2, k + 3 < kend);
-                KH_PROBE(2)
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
@@ -507,7 +486,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 }
                 if (STAGE == 2) { va[f] = s0[f * RAWF]; vb[f] = s0[f * RAWF + PTX]; }
             }
-            KH_PROBE(3)
             block_bar();
             // ---------------- phase C of plane k + phase A of plane k+1, as one block of straight-line code ----------
             // C: fp64 update of plane k, written in place, explicitly rounded so that the result
@@ -534,7 +512,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     below[f] = wt[f * WTF - (PTX + 4)].y;
                     above[f] = wt[f * WTF + (PTX + 4)].x;
                 }
-                KH_PROBE(4)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     // the state the flux differences are added to: the stage input (Heun), U^n (van Leer corrector)
@@ -579,7 +556,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     plm_m<MODE>(mk(below[f], q.x), q, mk(q.y, above[f]), qLy[f], QRy[f]);
                     QLyo[f] = qLy[f].x;
                 }
-                KH_PROBE(5)
                 if (MODE == 1) {
                     // W^{n+1/2} as float_t primitives (actual pressure: offset 0), written as a float box [5][PTY][PTX]
                     // over the head of the raw plane just consumed (every thread read its entries before barrier 2)
@@ -609,7 +585,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     qly[f * QYF + PTX] = qLy[f].y;
                 }
                 fence_async_smem();  // the producer ships the updated box after the next barrier
-                KH_PROBE(6)
             }
             // rotate the z march and the ring
 #pragma unroll
@@ -702,7 +677,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     const float pref_f = (float)pref_d;
 #pragma unroll
                     for (int f = 0; f < 5; f++) { W0[f] = sf[f * 2 * PTX + hsd.idx0 * PTX]; W1[f] = sf[f * 2 * PTX + hsd.idx1 * PTX]; }
-                    W0[1] = __fadd_rn(W0[1], -pref_f); W1[1] = __fadd_rn(W1[1], -pref_f);
+                    W0[1] = pdev(W0[1], pref_f); W1[1] = pdev(W1[1], pref_f);
                     W0[3] = apply_vn_rule(W0[3], ry);  W1[3] = apply_vn_rule(W1[3], ry);
                 } else {
                 double u0[5], u1[5];
@@ -767,7 +742,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     const float pref_f = (float)pref_d;
 #pragma unroll
                     for (int f = 0; f < 5; f++) { Wa[f] = sf[f * PTY * 4]; Wb[f] = sf[f * PTY * 4 + 4]; }
-                    Wa[1] = __fadd_rn(Wa[1], -pref_f); Wb[1] = __fadd_rn(Wb[1], -pref_f);
+                    Wa[1] = pdev(Wa[1], pref_f); Wb[1] = pdev(Wb[1], pref_f);
                     Wa[2] = apply_vn_rule(Wa[2], rx);  Wb[2] = apply_vn_rule(Wb[2], rx);
                 } else {
                 double ua[5], ub[5];
@@ -884,15 +859,6 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
     }
     }
 
-#ifdef KH_TMA_TIMING
-    if (blockIdx.x == 3 && blockIdx.y == 5 && blockIdx.z == 1 && lane == 0) {
-        if (warp == 0)
-            printf("stage %d warp 0 segments: gather %lld riemann %lld recover %lld accumulate %lld | loads %lld compute %lld stores %lld\n",
-                   STAGE, bt.seg[0], bt.seg[1], bt.seg[2], bt.seg[3], bt.seg[4], bt.seg[5], bt.seg[6]);
-        printf("stage %d warp %2d: barriers %d | before bar1: work %lld wait %lld | before bar2: work %lld wait %lld\n", STAGE, warp,
-               bt.n, bt.work[0], bt.wait[0], bt.work[1], bt.wait[1]);
-    }
-#endif
     if (hits) atomicAdd(&ctrl->floor_hits, (unsigned long long)hits);
     if (STAGE == 2) {
         __syncthreads();

@@ -1,0 +1,55 @@
+"""Comparison metrics of the GPU parity tests (CUDA path against the fp64 CPU oracle).
+
+Two bounds per conserved field f (BASELINE.json north_star + DESIGN.md section 7):
+
+* relative L1:  sum |f_gpu - f_orc| / sum |f_orc|  <=  1e-5 (mixed precision), 1e-12 (all-fp64);
+* pointwise:    max |f_gpu - f_orc| / scale(f)     <=  1e-4 (mixed),           1e-11 (all-fp64),
+  scale(f) = max(max f_orc - min f_orc, 0.1 max |f_orc|): the field's range, or a tenth of its
+  magnitude where the field is nearly uniform (fp32 rounding errors scale with the magnitude).
+  One wrong cell in a block of 10^4 moves the L1 sum by 10^-4 of its own error and would pass the
+  first bound; it cannot pass this one.  Measured on the five BASELINE configs at full size
+  (profiles/r2_parity_full_size.md): <= 9.2e-6 mixed, <= 8.4e-14 all-fp64.
+
+Fields that are identically zero in the oracle (unused momenta) must be identically zero on the GPU.
+"""
+import numpy as np
+
+MIXED, FP64 = 0, 1
+TOL_L1 = {MIXED: 1e-5, FP64: 1e-12}
+TOL_MAX = {MIXED: 1e-4, FP64: 1e-11}
+
+
+def rel_l1_fields(got, ref):
+    """Per-field relative L1; fields identically zero in the oracle must be identically zero."""
+    out = []
+    for m in range(5):
+        den = np.abs(ref[m]).sum()
+        if den == 0.0:
+            assert np.all(got[m] == 0.0), f"field {m} must stay exactly zero"
+            out.append(0.0)
+        else:
+            out.append(float(np.abs(got[m] - ref[m]).sum() / den))
+    return out
+
+
+def field_scale(ref_m):
+    return max(float(ref_m.max() - ref_m.min()), 0.1 * float(np.abs(ref_m).max()))
+
+
+def max_norm_fields(got, ref):
+    """Per-field max |got - ref| / scale(ref); 0 for fields that are identically zero in the oracle."""
+    out = []
+    for m in range(5):
+        s = field_scale(ref[m])
+        out.append(0.0 if s == 0.0 else float(np.abs(got[m] - ref[m]).max() / s))
+    return out
+
+
+def assert_parity(got, ref, prec, what="", tol_l1=None, tol_max=None):
+    """Both bounds, every field; NaN anywhere fails.  Returns (l1, maxnorm) per field for reporting."""
+    assert np.isfinite(got).all(), f"{what}: non-finite values in the GPU state"
+    l1 = rel_l1_fields(got, ref)
+    mx = max_norm_fields(got, ref)
+    assert max(l1) <= (TOL_L1[prec] if tol_l1 is None else tol_l1), (what, "rel-L1", l1)
+    assert max(mx) <= (TOL_MAX[prec] if tol_max is None else tol_max), (what, "max-norm", mx)
+    return l1, mx

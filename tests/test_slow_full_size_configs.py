@@ -1,0 +1,195 @@
+"""The five BASELINE.json configurations at their stated size and step count, CUDA path (through the C-ABI, the
+kernel and slab height `auto` picks = what bench.py times) against the fp64 CPU oracle, in mixed precision
+(rel-L1 <= 1e-5 per field) and all-fp64 mode (<= 1e-12), each with the pointwise bound of parity_utils.
+
+    C1  256-cell two-state problems, seeds 1..32, Free boundaries, gamma 1.4, to t = 0.2
+    C2  512^2 advected density wave, periodic, gamma 5/3, one full period (t = 1, about 6 250 steps)
+    C3  2048^2 shear layer, periodic, 100 steps
+    C4  256^3 point blast, Outflow boundaries, 50 steps, no floor activation on either side
+    C5  512^3 decaying turbulence, periodic, gamma 1.001, 20 steps: sampled sub-blocks the oracle recomputes
+        from their full domain of dependence, plus the same recipe at 256^3 compared cell by cell
+
+Minutes of oracle time on the host cores (C2 and C4 about two minutes each): marked `slow`.  The file name sorts
+last so that the quick parity matrix runs first.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2501_02317_b200 import binding, inputs
+from parity_utils import FP64, MIXED, assert_parity
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+F = inputs.FREE
+
+
+def gpu_run(pr, prec, until=None, kernel=binding.KERNEL_AUTO):
+    nx, ny, nz = pr.shape
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=prec, kernel=kernel)
+    h.set_state(pr.U)
+    T0 = h.totals()
+    if until is not None:
+        t, n = h.run_until(pr.cfl, until)
+    else:
+        t, n = h.run(pr.cfl, pr.nsteps), pr.nsteps
+    h.status()
+    Ug, T1, hits = h.get_state(), h.totals(), h.floor_hits()
+    h.destroy()
+    return Ug, t, n, hits, T0, T1
+
+
+def drift(T0, T1, U):
+    A0 = np.array([math.fsum(np.abs(U[m]).ravel()) for m in range(5)])
+    return float((np.abs(T1 - T0) / np.maximum(np.maximum(np.abs(T0), A0), 1e-300)).max())   # (unused momenta: 0 / tiny)
+
+
+# --------------------------------------------------------------------------- C1
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+@pytest.mark.parametrize("seed", range(1, 33))
+def test_c1_all_seeds(seed, prec):
+    pr = inputs.riemann_1d(seed, 256)
+    Uo = pr.U.copy()
+    to, no, hits_o = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 10 ** 6, 0.0, 0.2)
+    Ug, tg, ng, hits, _, _ = gpu_run(pr, prec, until=0.2)
+    assert hits == 0 and hits_o == 0
+    assert tg == pytest.approx(0.2, abs=1e-15)
+    assert abs(ng - no) <= (0 if prec == FP64 else 1)
+    assert_parity(Ug, Uo, prec, what=f"C1 seed {seed}")
+
+
+# --------------------------------------------------------------------------- C2
+@pytest.fixture(scope="module")
+def c2_oracle():
+    pr = inputs.advected_wave_2d(512, t_end=1.0)
+    Uo = pr.U.copy()
+    to, no, hits = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 10 ** 7, 0.0, 1.0)
+    assert to == 1.0 and hits == 0
+    return pr, Uo, no
+
+
+def eq6_l1(q, q0):
+    """Eq. 6: sum |q - q0| / (N [max q0 - min q0])."""
+    return float(np.abs(q - q0).sum() / (q0.size * (q0.max() - q0.min())))
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c2_full_period(c2_oracle, prec):
+    pr, Uo, no = c2_oracle
+    Ug, tg, ng, hits, T0, T1 = gpu_run(pr, prec, until=1.0)
+    assert tg == 1.0 and hits == 0
+    assert abs(ng - no) <= (0 if prec == FP64 else 2)
+    assert_parity(Ug, Uo, prec, what="C2 512^2, one period")
+    assert drift(T0, T1, pr.U) <= 1e-13
+    # back at the initial state after one crossing time: the Eq. 6 error of the density is the
+    # scheme's own truncation error, the same number on both sides, and falls as ~N^-2 (the oracle
+    # alone gives 1.98e-2, 5.55e-3, 1.53e-3 at N = 64, 128, 256 for this diagonal wave: a factor 3.6 per doubling)
+    e_gpu, e_orc = eq6_l1(Ug[0], pr.U[0]), eq6_l1(Uo[0], pr.U[0])
+    assert e_gpu == pytest.approx(e_orc, rel=1e-3 if prec == MIXED else 1e-9)
+    assert e_gpu < 1.53e-3 / 3.0
+
+
+# --------------------------------------------------------------------------- C3
+@pytest.fixture(scope="module")
+def c3_oracle():
+    pr = inputs.shear_layer_2d(2048, seed=3, nsteps=100)
+    Uo = pr.U.copy()
+    _, _, hits = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 100)
+    assert hits == 0
+    return pr, Uo
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c3_full_size(c3_oracle, prec):
+    pr, Uo = c3_oracle
+    Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
+    assert hits == 0
+    assert_parity(Ug, Uo, prec, what="C3 2048^2, 100 steps")
+    assert drift(T0, T1, pr.U) <= 1e-13
+
+
+# --------------------------------------------------------------------------- C4
+@pytest.fixture(scope="module")
+def c4_oracle():
+    pr = inputs.point_blast_3d(256, nsteps=50)
+    Uo = pr.U.copy()
+    _, _, hits = oracle.run(Uo, pr.gamma, pr.bc, 0.4, 50)
+    assert hits == 0          # PAPER.md Sec. 4.7 shape: no floor may fire on the oracle side either
+    return pr, Uo
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c4_full_size(c4_oracle, prec):
+    pr, Uo = c4_oracle
+    Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
+    assert hits == 0
+    assert_parity(Ug, Uo, prec, what="C4 256^3, 50 steps")
+    # the ambient gas at the edges is still at rest: mass and energy leave through no face
+    assert abs(T1[0] - T0[0]) <= 1e-13 * T0[0] and abs(T1[4] - T0[4]) <= 1e-13 * T0[4]
+
+
+# --------------------------------------------------------------------------- C5
+@pytest.fixture(scope="module")
+def c5_256_oracle():
+    pr = inputs.turbulence_3d(256, seed=5, nsteps=20)
+    Uo = pr.U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 20)
+    return pr, Uo
+
+
+@pytest.mark.parametrize("prec", [MIXED, FP64])
+def test_c5_recipe_at_256_cell_by_cell(c5_256_oracle, prec):
+    pr, Uo = c5_256_oracle
+    Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
+    assert hits == 0
+    assert_parity(Ug, Uo, prec, what="C5 recipe at 256^3, 20 steps")
+    assert drift(T0, T1, pr.U) <= 1e-13
+
+
+def test_c5_full_size_all_20_steps_sampled():
+    """512^3, mixed precision, the TMA kernel with its automatic slab height (bench.py's launch configuration), all
+    20 steps.  The oracle cannot run 512^3 x 20 in minutes, so it recomputes sampled 12^3 cores from the initial
+    state of their domain of dependence: 20 steps x 2 stages x 2 cells = 80 cells on every side (172^3 cells per
+    sample, Free boundaries on the sub-block, whose error cannot reach the core), with the dt sequence of the GPU
+    run.  Each dt is the GPU's fp64 CFL reduction (test_cfl_dt_matches_oracle: equal to the oracle's to 1e-13; the
+    first one is checked against the oracle's own reduction over the full state).  Samples sit on tile seams, slab
+    seams, the periodic wrap and at random places."""
+    n, nstep, halo, core = 512, 20, 80, 12
+    try:
+        pr = inputs.turbulence_3d(n, seed=5, nsteps=nstep)
+    except MemoryError:
+        pytest.skip("not enough host memory for the 512^3 state")
+    h = binding.KratosHydro(n, n, n, pr.gamma, pr.bc, precision=MIXED)
+    h.set_state(pr.U)
+    T0 = h.totals()
+    dts = []
+    for _ in range(nstep):
+        dts.append(h.cfl_dt(0.4))
+        h.step(dts[-1])
+    h.status()
+    T1 = h.totals()
+    Ug = h.get_state()
+    assert h.floor_hits() == 0
+    h.destroy()
+    assert drift(T0, T1, pr.U) <= 1e-13
+    assert dts[0] == pytest.approx(oracle.cfl_dt(pr.U, pr.gamma, 0.4), rel=1e-13)
+    rng = np.random.default_rng(2025)
+    w = core + 2 * halo
+    # (k0, j0, i0) of the cores: block corner across the periodic wrap; a 32 x 16 tile corner on a slab seam
+    # (the automatic slab height divides 512 into equal parts: plane 256 starts a slab for every power of two);
+    # two random places
+    corners = [(n - 6, n - 6, n - 6), (256 - 6, 16 * 9 - 6, 32 * 5 - 6)]
+    corners += [tuple(int(c) for c in rng.integers(0, n, 3)) for _ in range(2)]
+    for (k0, j0, i0) in corners:
+        kk = np.arange(k0 - halo, k0 - halo + w) % n
+        jj = np.arange(j0 - halo, j0 - halo + w) % n
+        ii = np.arange(i0 - halo, i0 - halo + w) % n
+        sub = np.ascontiguousarray(pr.U[:, kk][:, :, jj][:, :, :, ii])
+        for dt in dts:
+            oracle.step(sub, pr.gamma, (F,) * 6, dt, spacing=(1.0 / n,) * 3)
+        ref = sub[:, halo:halo + core, halo:halo + core, halo:halo + core]
+        kc, jc, ic = np.arange(k0, k0 + core) % n, np.arange(j0, j0 + core) % n, np.arange(i0, i0 + core) % n
+        got = Ug[:, kc][:, :, jc][:, :, :, ic]
+        assert_parity(got, ref, MIXED, what=f"C5 512^3 core at {(k0, j0, i0)}")
