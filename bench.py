@@ -47,6 +47,10 @@ def workload(name: str):
         return inputs.turbulence_3d(128, seed=5, nsteps=20), "C5 recipe at 128^3"
     if name == "C4":
         return inputs.point_blast_3d(256, nsteps=50), "C4 3D point blast 256^3 outflow gamma=5/3"
+    if name == "C1":
+        return inputs.riemann_1d(1, 256), "C1 1D two-state problem, 256 cells, Free boundaries, gamma=1.4 (seed 1)"
+    if name == "C2":
+        return inputs.advected_wave_2d(512), "C2 2D advected density wave 512^2 periodic gamma=5/3"
     if name == "C3":
         return inputs.shear_layer_2d(2048, seed=3, nsteps=100), "C3 2D shear layer 2048^2 periodic gamma=5/3"
     if name == "implosion":

@@ -40,8 +40,14 @@ using tma::halo_side;
 
 constexpr int SW = 28;        // columns of output per warp (lanes 2..29 of the 32-lane window)
 constexpr int NRING = 5;      // row pairs in flight per warp: p-1 (update), p, p+1 (converted ahead), p+2, p+3 (arriving)
-constexpr int WARPS = 4;      // warps per block (independent of each other)
-constexpr int BLOCKS_PER_SM = 3;
+#ifndef KH_STRIP_WARPS
+#define KH_STRIP_WARPS 4
+#endif
+#ifndef KH_STRIP_BLOCKS
+#define KH_STRIP_BLOCKS 3
+#endif
+constexpr int WARPS = KH_STRIP_WARPS;           // warps per block (independent of each other)
+constexpr int BLOCKS_PER_SM = KH_STRIP_BLOCKS;  // 12 warps per SM at <= 168 registers
 constexpr unsigned BOX_BYTES = 5 * 2 * 32 * 8;   // 2560
 constexpr unsigned HBOX_BYTES = 5 * 2 * 2 * 8;   // 160
 
@@ -124,69 +130,81 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
     }
     __syncwarp();
 
-    // pair q (rows 2q, 2q+1; q in [-1, npair]) -> the box rows that hold it (Sec. 3.1.1 in y)
-    auto issue = [&](int q) {   // lane 0
-        const HaloSide ys = halo_side(2 * q, ny, g.bc[2], g.bc[3]);
-        const int slot = (q + NRING) % NRING;
+    // pair q (rows 2q, 2q+1; q in [-1, npair]) -> the box rows that hold it (Sec. 3.1.1 in y).  Interior pairs are
+    // their own source; the two ghost pairs of the block take theirs from where the boundary rule says.
+    const HaloSide ylo = halo_side(-2, ny, g.bc[2], g.bc[3]);
+    const HaloSide yhi = halo_side(ny, ny, g.bc[2], g.bc[3]);
+    const unsigned tx_bytes = BOX_BYTES + (need_lo ? HBOX_BYTES : 0u) + (need_hi ? HBOX_BYTES : 0u);
+    auto issue = [&](int q, int slot) {   // lane 0
+        const int row = (q < 0) ? ylo.start : ((q >= npair) ? yhi.start : 2 * q);
         unsigned long long* bar = &sm.full[slot];
-        tma::mbar_expect_tx(bar, BOX_BYTES + (need_lo ? HBOX_BYTES : 0u) + (need_hi ? HBOX_BYTES : 0u));
-        tma_load3(&sm.raw[slot][0][0][0], &maps.in_own, x0 - 2, ys.start, 0, bar);
-        if (need_lo) tma_load3(&sm.hx[slot][0][0], &maps.in_cols, xlo.start, ys.start, 0, bar);
-        if (need_hi) tma_load3(&sm.hx[slot][1][0], &maps.in_cols, xhi.start, ys.start, 0, bar);
+        tma::mbar_expect_tx(bar, tx_bytes);
+        tma_load3(&sm.raw[slot][0][0][0], &maps.in_own, x0 - 2, row, 0, bar);
+        if (need_lo) tma_load3(&sm.hx[slot][0][0], &maps.in_cols, xlo.start, row, 0, bar);
+        if (need_hi) tma_load3(&sm.hx[slot][1][0], &maps.in_cols, xhi.start, row, 0, bar);
     };
-    // The ring is indexed by (q mod NRING); each slot's mbarrier flips once per use.
-    unsigned phase_bits = 0u;   // bit `slot`: parity to wait for next
+    // Each slot's mbarrier flips once per use: bit `slot` of phase_bits is the parity to wait for next.
+    unsigned phase_bits = 0u;
     int hits = 0;
-    auto convert = [&](int q, f2 W[5], bool count) {
-        const HaloSide ys = halo_side(2 * q, ny, g.bc[2], g.bc[3]);
-        const int slot = (q + NRING) % NRING;
+    auto convert = [&](int q, int slot, f2 (&W)[5], bool count) {
+        int i0 = 0, i1 = 1, ry = VN_KEEP;
+        if (q < 0) { i0 = ylo.idx0; i1 = ylo.idx1; ry = ylo.rule; }
+        else if (q >= npair) { i0 = yhi.idx0; i1 = yhi.idx1; ry = yhi.rule; }
         tma::mbar_wait_parity(&sm.full[slot], (phase_bits >> slot) & 1u);
         phase_bits ^= 1u << slot;
         double ua[5], ub[5];
         if (from_ghost_box) {
             const double* b = hx_base + slot * (2 * 32);
 #pragma unroll
-            for (int f = 0; f < 5; f++) { ua[f] = b[f * 4 + ys.idx0 * 2]; ub[f] = b[f * 4 + ys.idx1 * 2]; }
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 4 + i0 * 2]; ub[f] = b[f * 4 + i1 * 2]; }
         } else {
             const double* b = own_base + slot * (5 * 2 * 32);
 #pragma unroll
-            for (int f = 0; f < 5; f++) { ua[f] = b[f * 64 + ys.idx0 * 32]; ub[f] = b[f * 64 + ys.idx1 * 32]; }
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 64 + i0 * 32]; ub[f] = b[f * 64 + i1 * 32]; }
         }
         float Wa[5], Wb[5];
-        const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, ys.rule, VN_KEEP, Wa);
-        const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, ys.rule, VN_KEEP, Wb);
+        const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, ry, VN_KEEP, Wa);
+        const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, ry, VN_KEEP, Wb);
         if (count && owner) hits += ha + hb;
 #pragma unroll
         for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
     };
 
-    // ---- prologue: pairs pbeg-1 .. pbeg+2 in flight, W(pbeg-1) and W(pbeg) converted ----
+    // ---- prologue: pairs pbeg-1 .. pbeg+2 in flight (slots 0..3), W(pbeg-1) and W(pbeg) converted ----
     if (lane == 0)
-        for (int q = pbeg - 1; q <= min(pbeg + 2, pend); q++) issue(q);
-    f2 Wm[5], W0[5], Wp[5];
-    convert(pbeg - 1, Wm, false);
-    convert(pbeg, W0, true);
+        for (int q = pbeg - 1; q <= min(pbeg + 2, pend); q++) issue(q, q - (pbeg - 1));
+    f2 WA[5], WB[5];              // W(p) and W(p+1), swapping roles from trip to trip
+    float Wmy[5];                 // upper row of pair p-1
     float QLc[5];                 // left state of the y face below row 2p (limited state of row 2p-1 at its upper face)
-    double2 dUprev[5];            // flux sums of pair p-1: row 2p-2 complete, row 2p-1 lacks the face above it
+    double pend_y[5];             // flux sum of row 2p-1, lacking the face above it (which trip p solves)
+    {
+        f2 Wm[5];
+        convert(pbeg - 1, 0, Wm, false);
+        convert(pbeg, 1, WA, true);
 #pragma unroll
-    for (int f = 0; f < 5; f++) {
-        f2 qL, qR;
-        plm(mk(Wm[f].x, Wm[f].x), Wm[f], mk(Wm[f].y, W0[f].x), qL, qR);   // row 2pbeg-1 from rows 2pbeg-2, 2pbeg-1, 2pbeg
-        QLc[f] = qL.y;
-        dUprev[f] = make_double2(0.0, 0.0);
+        for (int f = 0; f < 5; f++) {
+            f2 qL, qR;
+            plm(mk(Wm[f].x, Wm[f].x), Wm[f], mk(Wm[f].y, WA[f].x), qL, qR);   // row 2pbeg-1 from rows 2pbeg-2, 2pbeg-1, 2pbeg
+            QLc[f] = qL.y;
+            Wmy[f] = Wm[f].y;
+            pend_y[f] = 0.0;
+        }
     }
     const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1];
     const CflConst<float> cc(g);
     f2 rate = mk(0.0f, 0.0f);
     const long long col_off = (long long)(owner ? c : 0);
+    // ring slots of the pairs p-1 (row 2p-1 updated), p+1 (converted) and p+3 (issued) at trip p; pair p sits in s_upd + 1
+    int s_upd = 0, s_conv = 2, s_issue = 4;
 
-    // trip p solves the faces of pair p and completes the update of pair p-1; the last trip (p == pend) only completes
-#pragma unroll 1
-    for (int p = pbeg; p <= pend; p++) {
-        if (lane == 0 && p + 3 <= pend) issue(p + 3);    // into the slot pair p-2 left after its update in trip p-1
-        const bool upd = (p > pbeg) && owner;
-        const long long cell_prev = (long long)(2 * (p - 1)) * nx + col_off;
-        if (p + 1 <= pend) convert(p + 1, Wp, p + 1 < pend);
+    // Trip p solves the faces of pair p; that completes row 2p-1 (the face above it was missing) and row 2p, which are
+    // updated and stored; row 2p+1 waits for the next trip.  The first trip of a slab stores row 2p only, the last one
+    // (p == pend) row 2p-1 only.  W0 = W(p) on entry, Wp receives W(p+1).
+    auto trip = [&](int p, f2 (&W0)[5], f2 (&Wp)[5]) {
+        if (lane == 0 && p + 3 <= pend) issue(p + 3, s_issue);    // into the slot pair p-2 left in trip p-1
+        const bool upd_a = (p > pbeg) && owner, upd_b = (p < pend) && owner;   // rows 2p-1, 2p
+        const long long cell_a = (long long)(2 * p - 1) * nx + col_off;        // row 2p-1; row 2p is + nx
+        if (p + 1 <= pend) convert(p + 1, s_conv, Wp, p + 1 < pend);
         // ---- slopes (Eq. 3) and the two face pairs of pair p ----
         f2 L[2][5], R[2][5], Fn[2][5];
         {
@@ -195,7 +213,8 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
             for (int f = 0; f < 5; f++) {
                 const f2 xm = shfl_up2(W0[f]), xp = shfl_down2(W0[f]);
                 plm(xm, W0[f], xp, qLx[f], qRx[f]);
-                plm(mk(Wm[f].y, W0[f].x), W0[f], mk(W0[f].y, Wp[f].x), qLy[f], qRy[f]);
+                plm(mk(Wmy[f], W0[f].x), W0[f], mk(W0[f].y, Wp[f].x), qLy[f], qRy[f]);
+                Wmy[f] = W0[f].y;
             }
             f2 t[5];
 #pragma unroll
@@ -208,48 +227,42 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
             tma::to_normal<1>(qRy, R[1]);
         }
         tma::hllc2n<2>(L, R, gas, Fn);
-        // U0 of pair p-1 for the Heun average: issued here, where the registers of the solver are free again; the other
-        // warps of the SM cover its latency
+        // U0 of the two rows for the Heun average: issued here, where the registers of the solver are free again; the
+        // other warps of the SM cover its latency
         double2 v0[5];
-        if (STAGE == 2 && upd) {
+        if (STAGE == 2) {
 #pragma unroll
-            for (int f = 0; f < 5; f++) v0[f] = make_double2(U0[f * N + cell_prev], U0[f * N + cell_prev + nx]);
+            for (int f = 0; f < 5; f++)
+                v0[f] = make_double2(upd_a ? U0[f * N + cell_a] : 0.0, upd_b ? U0[f * N + cell_a + nx] : 0.0);
         }
-        double2 dU[5];
+        double ua[5], ub[5];   // new state of rows 2p-1, 2p
         {
             f2 Fx[5], Fy[5];
             tma::from_normal<0>(Fn[0], Fx);
             tma::from_normal<1>(Fn[1], Fy);
+            const double* ba = own_base + s_upd * (5 * 2 * 32) + 32;                               // row 2p-1 in the ring
+            const double* bb = own_base + ((s_upd + 1 == NRING) ? 0 : s_upd + 1) * (5 * 2 * 32);   // row 2p
 #pragma unroll
             for (int f = 0; f < 5; f++) {
                 const f2 fxh = shfl_down2(Fx[f]);                          // flux through the face at c + 1/2
                 const double flo = (double)Fy[f].x, fin = (double)Fy[f].y;
-                // pair p: x faces of both rows, the y faces 2p-1/2 (+, row 2p) and 2p+1/2 (-, row 2p; +, row 2p+1)
-                dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin),
-                                   __dmul_rn(dtdx, __dadd_rn((double)Fx[f].x, -(double)fxh.x)));
-                dU[f].y = __fma_rn(dtdy, fin, __dmul_rn(dtdx, __dadd_rn((double)Fx[f].y, -(double)fxh.y)));
-                // pair p-1: its upper face is this pair's lower face
-                dUprev[f].y = __fma_rn(-dtdy, flo, dUprev[f].y);
-            }
-        }
-        // ---- fp64 update of pair p-1, in global memory order ----
-        if (upd) {
-            const int slot = (p - 1 + NRING) % NRING;
-            const double* b = own_base + slot * (5 * 2 * 32);
-            double ua[5], ub[5];
-#pragma unroll
-            for (int f = 0; f < 5; f++) {
-                double xa = __dadd_rn(b[f * 64], dUprev[f].x);
-                double xb = __dadd_rn(b[f * 64 + 32], dUprev[f].y);
+                // fp64 update.  Row 2p-1: its sum so far and the face above it (2p-1/2).
+                // Row 2p: x faces, y faces 2p-1/2 (+) and 2p+1/2 (-).  Row 2p+1 so far: x faces, y face 2p+1/2 (+).
+                double xa = __dadd_rn(ba[f * 64], __fma_rn(-dtdy, flo, pend_y[f]));
+                double xb = __dadd_rn(bb[f * 64], __fma_rn(dtdy, __dadd_rn(flo, -fin),
+                                                           __dmul_rn(dtdx, __dadd_rn((double)Fx[f].x, -(double)fxh.x))));
+                pend_y[f] = __fma_rn(dtdy, fin, __dmul_rn(dtdx, __dadd_rn((double)Fx[f].y, -(double)fxh.y)));
                 if (STAGE == 2) {
                     xa = __fma_rn(0.5, v0[f].x, __dmul_rn(0.5, xa));
                     xb = __fma_rn(0.5, v0[f].y, __dmul_rn(0.5, xb));
                 }
                 ua[f] = xa;
                 ub[f] = xb;
-                Uout[f * N + cell_prev] = xa;
-                Uout[f * N + cell_prev + nx] = xb;
+                if (upd_a) Uout[f * N + cell_a] = xa;
+                if (upd_b) Uout[f * N + cell_a + nx] = xb;
             }
+        }
+        {
             if (STAGE == 2) {   // CFL rate of the new state (readings S1/S7), both rows at once
                 using namespace pr;
                 const float rfl = (float)KH_RHO_FLOOR, pfl = (float)KH_P_FLOOR;
@@ -268,12 +281,18 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
                 rt = fma2(add2(mk(fabsf(vy.x), fabsf(vy.y)), cs), bc(cc.idy), rt);
                 if (!(rt.x == rt.x)) rt.x = __int_as_float(0x7f800000);
                 if (!(rt.y == rt.y)) rt.y = __int_as_float(0x7f800000);
-                rate = mk(fmaxf(rate.x, rt.x), fmaxf(rate.y, rt.y));
+                rate = mk(upd_a ? fmaxf(rate.x, rt.x) : rate.x, upd_b ? fmaxf(rate.y, rt.y) : rate.y);
             }
         }
         __syncwarp();   // every lane has read pair p-1 from the ring before lane 0 refills that slot in the next trip
-#pragma unroll
-        for (int f = 0; f < 5; f++) { Wm[f] = W0[f]; W0[f] = Wp[f]; dUprev[f] = dU[f]; }
+        if (++s_upd == NRING) s_upd = 0;
+        if (++s_conv == NRING) s_conv = 0;
+        if (++s_issue == NRING) s_issue = 0;
+    };
+#pragma unroll 1
+    for (int p = pbeg; p <= pend; p += 2) {   // two trips per turn: the two register sets swap roles instead of being copied
+        trip(p, WA, WB);
+        if (p + 1 <= pend) trip(p + 1, WB, WA);
     }
 
     if (hits) atomicAdd(&ctrl->floor_hits, (unsigned long long)hits);
@@ -322,11 +341,18 @@ inline void build_maps(StageMaps* sm, const double* A, const double* B, const Gr
 
 inline int auto_rows(const Grid& g)
 {
-    // >= ~4 waves of warps over 148 SMs x 12 warps; slabs of >= 16 rows (every slab converts two extra pairs)
+    // One wave of equal work items: every SM holds BLOCKS_PER_SM x WARPS warps, each marching through one slab from
+    // the start of the kernel to its end, so that the prologue of a slab (two extra row pairs converted, the first box
+    // awaited) is paid once per warp.  Slabs shorter than 16 rows are not worth their prologue: small blocks then
+    // simply leave SMs idle (they are launch-bound anyway).
     const long long nstrips = (g.n[0] + SW - 1) / SW;
-    int rows = g.n[1];
-    while (rows > 16 && nstrips * ((g.n[1] + rows - 1) / rows) < 148LL * WARPS * BLOCKS_PER_SM * 4) rows = ((rows / 2) + 1) & ~1;
-    return rows;
+    const long long slots = 148LL * WARPS * BLOCKS_PER_SM;
+    long long nslabs = slots / nstrips;
+    if (nslabs < 1) nslabs = 1;
+    int rows = (int)((g.n[1] + nslabs - 1) / nslabs);
+    rows = (rows + 1) & ~1;
+    if (rows < 16) rows = 16;
+    return rows < g.n[1] ? rows : g.n[1];
 }
 
 inline void configure()
