@@ -118,6 +118,14 @@ __device__ __forceinline__ double fma_(double a, double b, double c) { return __
 // c = sqrt(gamma p / rho).  fp32: gamma p * rsqrt(gamma p rho), a single MUFU.
 __device__ __forceinline__ float sound_speed(float gp, float rho) { return mul_(gp, rsqrt_(mul_(gp, rho))); }
 __device__ __forceinline__ double sound_speed(double gp, double rho) { return sqrt(gp / rho); }
+// 1/p for the pressure ratio of Eq. 5.  fp32: t = rsqrt(gamma p rho) is the factor of the sound speed above and
+// 1/p = gamma rho t^2 (multiplications instead of another MUFU; the packed kernels do the same, bit for bit).
+__device__ __forceinline__ float inv_pressure(float gamma, float gp, float rho, float p)
+{
+    const float t = rsqrt_(mul_(gp, rho));
+    return mul_(mul_(gamma, rho), mul_(t, t));
+}
+__device__ __forceinline__ double inv_pressure(double gamma, double gp, double rho, double p) { return 1.0 / p; }
 
 // ---------------------------------------------------------------------------------------
 // Primitive state in a face-normal frame: u normal, v and w tangential.
@@ -214,8 +222,8 @@ __device__ __forceinline__ void hllc(const Prim<T>& L, const Prim<T>& R, const G
     T pst = fma_(T(-0.125), w, mul_(T(0.5), add_(L.p, R.p)));
     pst = fmax(pst, -gc.pref);
 
-    const T qL = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, L.p), rcp_(pL)), T(0)), T(1)));
-    const T qR = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, R.p), rcp_(pR)), T(0)), T(1)));
+    const T qL = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, L.p), inv_pressure(gc.gamma, mul_(gc.gamma, pL), L.r, pL)), T(0)), T(1)));
+    const T qR = sqrt_(fma_(gc.g1, fmax(mul_(sub_(pst, R.p), inv_pressure(gc.gamma, mul_(gc.gamma, pR), R.r, pR)), T(0)), T(1)));
     const T dsL = -mul_(cL, qL);
     const T dsR = mul_(cR, qR);
     const T mL = mul_(L.r, dsL);

@@ -83,14 +83,16 @@ __device__ __forceinline__ void hllc2(const f2 L[5], const f2 R[5], const Gas& g
     const f2 pref = bc(g.pref);
     const f2 pL = add2(L[1], pref), pR = add2(R[1], pref);
     const f2 gpL = mul2(bc(g.gamma), pL), gpR = mul2(bc(g.gamma), pR);
-    const f2 cL = mul2(gpL, rsqrt2(mul2(gpL, L[0])));
-    const f2 cR = mul2(gpR, rsqrt2(mul2(gpR, R[0])));
+    const f2 tL = rsqrt2(mul2(gpL, L[0])), tR = rsqrt2(mul2(gpR, R[0]));
+    const f2 cL = mul2(gpL, tL), cR = mul2(gpR, tR);
     const f2 w = mul2(mul2(sub2(R[2], L[2]), add2(L[0], R[0])), add2(cL, cR));
     f2 pst = fma2(bc(-0.125f), w, mul2(bc(0.5f), add2(L[1], R[1])));
     pst = maxs(pst, -g.pref);
     const f2 one = bc(1.0f);
-    const f2 qL = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst, L[1]), rcp2(pL))), one));
-    const f2 qR = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst, R[1]), rcp2(pR))), one));
+    // 1/p_K = gamma rho_K t_K^2 with t_K = rsqrt(gamma p_K rho_K) from the sound speed (see tma::hllc2n)
+    const f2 ipL = mul2(mul2(bc(g.gamma), L[0]), mul2(tL, tL)), ipR = mul2(mul2(bc(g.gamma), R[0]), mul2(tR, tR));
+    const f2 qL = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst, L[1]), ipL)), one));
+    const f2 qR = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst, R[1]), ipR)), one));
     const f2 dsL = neg2(mul2(cL, qL));
     const f2 dsR = mul2(cR, qR);
     const f2 mL = mul2(L[0], dsL), mR = mul2(R[0], dsR);
@@ -166,7 +168,11 @@ __device__ __forceinline__ int recover(double rho, double mx, double my, double 
     // (m.m)/rho with m.m formed first: it does not wait for the reciprocal, which shortens the dependent chain
     const double m2 = __dmul_rn(__fma_rn(mz, mz, __fma_rn(my, my, __dmul_rn(mx, mx))), ir);
     double p = __dmul_rn(gm1, __fma_rn(-0.5, m2, e));
+#ifdef KH_NO_PREF_FLOOR
+    const double pfl = KH_P_FLOOR;
+#else
     const double pfl = fmax(KH_P_FLOOR, __dmul_rn(pref, 0x1p-22));
+#endif
     const bool lo_p = p < pfl;
     p = lo_p ? pfl : p;
     if (rx | ry | rz) {

@@ -146,7 +146,11 @@ __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commi
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+#ifdef KH_WHATIF_NOBAR   // timing experiment only (wrong results): how much do the block barriers cost?
+__device__ __forceinline__ void block_bar() { __syncwarp(); }
+#else
 __device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "memory"); }
+#endif
 
 // Stored pressure deviation of a float_t primitive (van Leer corrector): p - pref with the same two-ulp floor as
 // pr::recover, so that the pressure rebuilt by the Riemann solver stays > 0.
@@ -177,13 +181,22 @@ __device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_h
 // lock step: every statement is issued for all N before the next one, so that the N dependency chains are
 // interleaved in program order and the fixed latencies of one hide behind the others.  Operation for operation
 // the same arithmetic as pr::hllc2, hence the same bits.
+// 1/p_K for the pressure ratio of Eq. 5.  t = rsqrt(gamma p rho) is at hand from the sound speed, and 1/p = gamma rho t^2:
+// three packed multiplications instead of two more MUFU operations per face pair (the XU pipe, which also carries the
+// fp32 <-> fp64 conversions, is the busiest one of this kernel).  A few ulp of error in a factor that only enters
+// through max(p*/p_K - 1, 0).
+#ifndef KH_RCP_MUFU
+#define KH_RCP_P(p, rho, t) mul2(mul2(bc(g.gamma), rho), mul2(t, t))
+#else
+#define KH_RCP_P(p, rho, t) rcp2(p)
+#endif
 template <int N>
 __device__ __forceinline__ void hllc2n(const f2 (&L)[N][5], const f2 (&R)[N][5], const Gas& g, f2 (&F)[N][5])
 {
     using namespace pr;
     const f2 pref = bc(g.pref), one = bc(1.0f);
 #define KH_EACH for (int n = 0; n < N; n++)
-    f2 pL[N], pR[N], gpL[N], gpR[N], cL[N], cR[N], w[N], pst[N], qL[N], qR[N], dsL[N], dsR[N], mL[N], mR[N];
+    f2 pL[N], pR[N], gpL[N], gpR[N], tL[N], tR[N], cL[N], cR[N], w[N], pst[N], qL[N], qR[N], dsL[N], dsR[N], mL[N], mR[N];
     f2 num[N], den[N], sL[N], rK[N], pKd[N], uK[N], vK[N], wK[N], dsK[N], mK[N], pK[N], sK[N], D[N], r[N];
     f2 sst[N], inv[N], ke[N], EK[N], phi[N], pstKd[N], F0[N], F1[N], A4[N], F4[N], G0[N], G1[N], G4[N];
     bool lx[N], ly[N], ox[N], oy[N];
@@ -192,15 +205,17 @@ __device__ __forceinline__ void hllc2n(const f2 (&L)[N][5], const f2 (&R)[N][5],
 #pragma unroll
     KH_EACH { gpL[n] = mul2(bc(g.gamma), pL[n]); gpR[n] = mul2(bc(g.gamma), pR[n]); }
 #pragma unroll
-    KH_EACH { cL[n] = mul2(gpL[n], rsqrt2(mul2(gpL[n], L[n][0]))); cR[n] = mul2(gpR[n], rsqrt2(mul2(gpR[n], R[n][0]))); }
+    KH_EACH { tL[n] = rsqrt2(mul2(gpL[n], L[n][0])); tR[n] = rsqrt2(mul2(gpR[n], R[n][0])); }
+#pragma unroll
+    KH_EACH { cL[n] = mul2(gpL[n], tL[n]); cR[n] = mul2(gpR[n], tR[n]); }
 #pragma unroll
     KH_EACH w[n] = mul2(mul2(sub2(R[n][2], L[n][2]), add2(L[n][0], R[n][0])), add2(cL[n], cR[n]));
 #pragma unroll
     KH_EACH pst[n] = maxs(fma2(bc(-0.125f), w[n], mul2(bc(0.5f), add2(L[n][1], R[n][1]))), -g.pref);
 #pragma unroll
     KH_EACH {
-        qL[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], L[n][1]), rcp2(pL[n]))), one));
-        qR[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], R[n][1]), rcp2(pR[n]))), one));
+        qL[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], L[n][1]), KH_RCP_P(pL[n], L[n][0], tL[n]))), one));
+        qR[n] = sqrt2(fma2(bc(g.g1), max0(mul2(sub2(pst[n], R[n][1]), KH_RCP_P(pR[n], R[n][0], tR[n]))), one));
     }
 #pragma unroll
     KH_EACH { dsL[n] = neg2(mul2(cL[n], qL[n])); dsR[n] = mul2(cR[n], qR[n]); }
