@@ -64,6 +64,9 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
  * Reconstruction is PLM-minmod and the Riemann solver HLLC (the paper's defaults; no other choice). */
 #define KRATOS_PREC_MIXED 0 /* float_t = fp32 (reconstruction, Riemann), float2_t = fp64 (state, update) */
 #define KRATOS_PREC_FP64 1  /* float_t = float2_t = fp64 */
+#define KRATOS_PREC_SINGLE 2 /* float_t = float2_t = fp32 ("Single" of Tables 1-2): the handle stores the state as
+                               floats (half the memory and traffic); the boundary still carries doubles, converted on the way in
+                               and out.  Conservation holds to fp32 rounding only.  Heun integrator only. */
 #define KRATOS_INTEGRATOR_HEUN (0 << 4)
 #define KRATOS_INTEGRATOR_VANLEER (1 << 4) /* predictor-corrector of Sec. 3.3: predictor kept as float_t
                                              primitives (20 B per cell in mixed precision instead of a second fp64 state);

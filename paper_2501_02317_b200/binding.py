@@ -16,7 +16,7 @@ import numpy as np
 
 from . import build as _build
 
-PREC_MIXED, PREC_FP64 = 0, 1
+PREC_MIXED, PREC_FP64, PREC_SINGLE = 0, 1, 2
 BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
 INTEGRATOR_HEUN, INTEGRATOR_VANLEER = 0 << 4, 1 << 4   # scheme word bits 4-5
 KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_TMA, KERNEL_STRIP = 0, 1, 2, 3, 5, 6

@@ -61,6 +61,7 @@ struct kratos_hydro {
     dd* partial;     // totals scratch (device)
     double* d_tot;   // 5 doubles (device)
     double* p_partial;  // per-block pressure sums of the cfl kernel (device)
+    double* stage_buf;  // Single mode: staging area for the double <-> float conversion of host states (device, on demand)
     int tot_blocks;
     cudaStream_t stream;
     int device;       // CUDA device the handle lives on (every entry point runs with it current)
@@ -138,6 +139,7 @@ void collect_timing(kratos_hydro* h)
 int auto_variant(const kratos_hydro* h)
 {
     if (h->integ == 1) return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;  // van Leer
+    if (h->prec == KRATOS_PREC_SINGLE) return KRATOS_KERNEL_SIMPLE;   // all-fp32 state: the general kernel
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
     if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
@@ -182,6 +184,22 @@ int launch_stage(kratos_hydro* h, int stage)
     return KRATOS_OK;
 }
 
+// All-fp32 "Single" mode: float2_t = float_t = float; both state arrays hold floats.
+int launch_stage_single(kratos_hydro* h, int stage)
+{
+    const Grid& g = h->g;
+    const float* A = reinterpret_cast<const float*>(h->U0);
+    float* B = reinterpret_cast<float*>(h->U1);
+    LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
+    const int threads = 128;
+    const long long blocks = (g.N + threads - 1) / threads;
+    if (stage == 1) stage_simple<float, 1, float><<<(unsigned)blocks, threads, 0, h->stream>>>(A, A, B, g, h->ctrl);
+    else            stage_simple<float, 2, float><<<(unsigned)blocks, threads, 0, h->stream>>>(B, A, const_cast<float*>(A), g, h->ctrl);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "stage %d launch: %s", stage, cudaGetErrorString(e));
+    return KRATOS_OK;
+}
+
 int launch_both_stages(kratos_hydro* h)
 {
     int rc;
@@ -198,6 +216,10 @@ int launch_both_stages(kratos_hydro* h)
             if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "van Leer sub-step %d launch: %s", which, cudaGetErrorString(e));
         }
         return KRATOS_OK;
+    }
+    if (h->prec == KRATOS_PREC_SINGLE) {
+        if ((rc = launch_stage_single(h, 1))) return rc;
+        return launch_stage_single(h, 2);
     }
     if (h->prec == KRATOS_PREC_MIXED) {
         if ((rc = launch_stage<float>(h, 1))) return rc;
@@ -217,7 +239,10 @@ int launch_cfl_rate(kratos_hydro* h)
         LaunchTimer lt(h, SLOT_OTHER);
         long long blocks = (h->g.N + 255) / 256;
         if (blocks > CFL_MAX_BLOCKS) blocks = CFL_MAX_BLOCKS;
-        cfl_rate_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl, h->p_partial);
+        if (h->prec == KRATOS_PREC_SINGLE)
+            cfl_rate_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>(reinterpret_cast<const float*>(h->U0), h->g, h->ctrl, h->p_partial);
+        else
+            cfl_rate_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>(h->U0, h->g, h->ctrl, h->p_partial);
         // the reference pressure is a function of the state given to set_state and of nothing else: calling
         // cfl_dt() between steps must not change what the following steps compute
         if (!h->pref_valid) {
@@ -248,6 +273,36 @@ int read_ctrl(kratos_hydro* h)
     return KRATOS_OK;
 }
 
+// Single mode: the boundary carries doubles, the handle stores floats.  Device buffers are converted directly; host
+// buffers go through a device staging area of at most 64 Mi doubles, chunk by chunk.  Synchronises for host buffers.
+int convert_state(kratos_hydro* h, double* U, int on_device, bool in)
+{
+    const long long n = 5 * h->g.N;
+    float* S = reinterpret_cast<float*>(h->U0);
+    const long long chunk = on_device ? n : (n < (64LL << 20) ? n : (64LL << 20));
+    if (!on_device && !h->stage_buf) CUDA_TRY(cudaMalloc(&h->stage_buf, sizeof(double) * (size_t)chunk));
+    for (long long o = 0; o < n; o += chunk) {
+        const long long m = (n - o < chunk) ? n - o : chunk;
+        double* dev = on_device ? U + o : h->stage_buf;
+        const unsigned blocks = (unsigned)((m + 255) / 256 < 148 * 16 ? (m + 255) / 256 : 148 * 16);
+        if (in) {
+            if (!on_device) CUDA_TRY(cudaMemcpyAsync(dev, U + o, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, h->stream));
+            LaunchTimer lt(h, SLOT_OTHER);
+            convert_state_kernel<double, float><<<blocks, 256, 0, h->stream>>>(dev, S + o, m);
+        } else {
+            {
+                LaunchTimer lt(h, SLOT_OTHER);
+                convert_state_kernel<float, double><<<blocks, 256, 0, h->stream>>>(S + o, dev, m);
+            }
+            if (!on_device) CUDA_TRY(cudaMemcpyAsync(U + o, dev, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, h->stream));
+        }
+        if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));   // the staging area is reused by the next chunk
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "state conversion: %s", cudaGetErrorString(e));
+    return KRATOS_OK;
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------
@@ -258,7 +313,7 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     if (!bc) { fail(KRATOS_ERR_ARG, "bc is NULL"); return nullptr; }
     if (!(gamma > 1.0) || !std::isfinite(gamma)) { fail(KRATOS_ERR_ARG, "gamma must be > 1"); return nullptr; }
     const int prec = scheme & 3, integ = (scheme >> 4) & 3;
-    if ((prec != KRATOS_PREC_MIXED && prec != KRATOS_PREC_FP64) || integ > 1 || (scheme & ~0x33)) {
+    if (prec > KRATOS_PREC_SINGLE || integ > 1 || (scheme & ~0x33) || (prec == KRATOS_PREC_SINGLE && integ != 0)) {
         fail(KRATOS_ERR_ARG, "unsupported scheme word 0x%x", scheme);
         return nullptr;
     }
@@ -321,7 +376,8 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->U0 = h->U1 = nullptr;
     h->ctrl = nullptr; h->h_ctrl = nullptr; h->partial = nullptr; h->d_tot = nullptr; h->p_partial = nullptr;
     h->tot_blocks = (int)((g.N + 255) / 256 < 592 ? (g.N + 255) / 256 : 592);
-    const size_t bytes = sizeof(double) * 5 * (size_t)g.N;
+    const size_t bytes = (prec == KRATOS_PREC_SINGLE ? sizeof(float) : sizeof(double)) * 5 * (size_t)g.N;
+    h->stage_buf = nullptr;
     // second array: the fp64 predictor of Heun, or the float_t primitives W^{n+1/2} of van Leer (PAPER.md:272:
     // "saves up to ~1/3 of the device memory": 40 + 20 instead of 40 + 40 bytes per cell in mixed precision)
     const size_t bytes1 = (integ == 1) ? (prec == KRATOS_PREC_MIXED ? sizeof(float) : sizeof(double)) * 5 * (size_t)g.N : bytes;
@@ -366,6 +422,7 @@ void kratos_hydro_destroy(kratos_hydro_t* h)
     cudaFree(h->partial);
     cudaFree(h->d_tot);
     cudaFree(h->p_partial);
+    cudaFree(h->stage_buf);
     if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
     delete h->maps;
     delete h->smaps;
@@ -395,6 +452,8 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
     if (variant == KRATOS_KERNEL_AUTO) variant = auto_variant(h);
+    if (h->prec == KRATOS_PREC_SINGLE && variant != auto_variant(h) && variant != KRATOS_KERNEL_SIMPLE)
+        return fail(KRATOS_ERR_ARG, "this kernel variant does not serve the all-fp32 mode on this block");
     if ((variant == KRATOS_KERNEL_TILED || variant == KRATOS_KERNEL_PAIRED) && !h->tiled_ok)
         return fail(KRATOS_ERR_ARG, "tiled and paired kernels need active x and y axes");
     if (variant == KRATOS_KERNEL_PAIRED && h->prec != KRATOS_PREC_MIXED)
@@ -422,8 +481,13 @@ int kratos_hydro_set_state(kratos_hydro_t* h, const double* U, int on_device)
     if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
     const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
     DeviceGuard dg(h);
-    CUDA_TRY(cudaMemcpyAsync(h->U0, U, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
-    if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (h->prec == KRATOS_PREC_SINGLE) {
+        int rc = convert_state(h, const_cast<double*>(U), on_device, true);
+        if (rc) return rc;
+    } else {
+        CUDA_TRY(cudaMemcpyAsync(h->U0, U, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+        if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
     h->rate_valid = false;
     h->pref_valid = false;
     return KRATOS_OK;
@@ -434,6 +498,7 @@ int kratos_hydro_get_state(kratos_hydro_t* h, double* U, int on_device)
     if (!h || !U) return fail(KRATOS_ERR_ARG, "NULL argument");
     const size_t bytes = sizeof(double) * 5 * (size_t)h->g.N;
     DeviceGuard dg(h);
+    if (h->prec == KRATOS_PREC_SINGLE) return convert_state(h, U, on_device, false);
     CUDA_TRY(cudaMemcpyAsync(U, h->U0, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
     if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
     return KRATOS_OK;
@@ -534,7 +599,10 @@ int kratos_hydro_totals(kratos_hydro_t* h, double out[5])
     DeviceGuard dg(h);
     {
         LaunchTimer lt(h, SLOT_OTHER);
-        totals_kernel<<<dim3(h->tot_blocks, 5), 256, 0, h->stream>>>(h->U0, h->g.N, h->partial);
+        if (h->prec == KRATOS_PREC_SINGLE)
+            totals_kernel<float><<<dim3(h->tot_blocks, 5), 256, 0, h->stream>>>(reinterpret_cast<const float*>(h->U0), h->g.N, h->partial);
+        else
+            totals_kernel<double><<<dim3(h->tot_blocks, 5), 256, 0, h->stream>>>(h->U0, h->g.N, h->partial);
     }
     {
         LaunchTimer lt(h, SLOT_OTHER);

@@ -157,6 +157,24 @@ __device__ __forceinline__ int cons_to_prim(double rho, double mx, double my, do
     return hits;
 }
 
+// All-fp32 "Single" mode (float2_t = float_t = float): the same recovery on an fp32 state, every
+// operation explicitly rounded (all copies of a cell return the same bits), 1/rho by MUFU.RCP.
+__device__ __forceinline__ int cons_to_prim(float rho, float mx, float my, float mz, float eps, float gm1, float& p,
+                                            float& vx, float& vy, float& vz, float& rho_out)
+{
+    int hits = 0;
+    if (rho < (float)KH_RHO_FLOOR) { rho = (float)KH_RHO_FLOOR; hits++; }
+    const float ir = rcp_(rho);
+    vx = mul_(mx, ir);
+    vy = mul_(my, ir);
+    vz = mul_(mz, ir);
+    const float m2 = mul_(fma_(mz, mz, fma_(my, my, mul_(mx, mx))), ir);
+    p = mul_(gm1, fma_(-0.5f, m2, eps));
+    if (p < (float)KH_P_FLOOR) { p = (float)KH_P_FLOOR; hits++; }
+    rho_out = rho;
+    return hits;
+}
+
 // Eq. 3, reading S2 for ab = 0: the argument of smaller magnitude when both have
 // the same sign, else 0.  fp32: FMNMX.XORSIGN gives min(|a|,|b|) carrying sign(a) xor sign(b); clamping
 // at 0 keeps it only for equal signs; the sign of a is put back with one LOP3 -- three ALU instructions.
@@ -288,8 +306,8 @@ struct CflConst {
         : gm1(T(g.gamma - 1.0)), gamma(T(g.gamma)), idx(T(g.inv_dx[0])), idy(T(g.inv_dx[1])), idz(T(g.inv_dx[2])) {}
 };
 
-template <typename T>
-__device__ __forceinline__ T cfl_rate_from_cons(const double Un[5], const CflConst<T>& cc, T* p_out = nullptr)
+template <typename T, typename S = double>
+__device__ __forceinline__ T cfl_rate_from_cons(const S Un[5], const CflConst<T>& cc, T* p_out = nullptr)
 {
     T r = T(Un[0]);
     r = (r < T(KH_RHO_FLOOR)) ? T(KH_RHO_FLOOR) : r;  // comparisons, not fmax: a NaN must survive

@@ -8,7 +8,9 @@ namespace kh {
 // Grid-stride, warp-shuffle + one atomicMax per block.  Also leaves each block's pressure sum in
 // p_partial[blockIdx.x] and its pressure minimum in p_partial[gridDim.x + blockIdx.x] (fixed reduction
 // order => run-to-run reproducible reference pressure).
-__global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict__ U, Grid g, Ctrl* ctrl,
+// S = float2_t, the storage type of the state (float in the all-fp32 Single mode: converted exactly to fp64 here).
+template <typename S>
+__global__ void __launch_bounds__(256) cfl_rate_kernel(const S* __restrict__ U, Grid g, Ctrl* ctrl,
                                                        double* p_partial)
 {
     __shared__ double red[32];
@@ -17,7 +19,7 @@ __global__ void __launch_bounds__(256) cfl_rate_kernel(const double* __restrict_
     const CflConst<double> cc(g);
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < g.N;
          c += (long long)gridDim.x * blockDim.x) {
-        const double u[5] = {U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c]};
+        const double u[5] = {(double)U[c], (double)U[g.N + c], (double)U[2 * g.N + c], (double)U[3 * g.N + c], (double)U[4 * g.N + c]};
         double p;
         double r = cfl_rate_from_cons<double>(u, cc, &p);
         if (!(r == r)) r = __longlong_as_double(0x7ff0000000000000LL);
@@ -112,15 +114,16 @@ __device__ __forceinline__ dd dd_add(dd a, dd b)
 }
 
 // partial[field][block] = double-double sum of that block's share.  Launch with 256 threads.
-__global__ void __launch_bounds__(256) totals_kernel(const double* __restrict__ U, long long N, dd* partial)
+template <typename S>
+__global__ void __launch_bounds__(256) totals_kernel(const S* __restrict__ U, long long N, dd* partial)
 {
     __shared__ dd red[8];
     const int field = blockIdx.y;
-    const double* f = U + (long long)field * N;
+    const S* f = U + (long long)field * N;
     dd acc{0.0, 0.0};
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < N;
          c += (long long)gridDim.x * blockDim.x)
-        acc = dd_add(acc, f[c]);
+        acc = dd_add(acc, (double)f[c]);
     for (int o = 16; o > 0; o >>= 1) {
         dd other{__shfl_xor_sync(0xffffffffu, acc.hi, o), __shfl_xor_sync(0xffffffffu, acc.lo, o)};
         acc = dd_add(acc, other);
@@ -133,6 +136,14 @@ __global__ void __launch_bounds__(256) totals_kernel(const double* __restrict__ 
         for (int w = 1; w < 8; w++) t = dd_add(t, red[w]);
         partial[(long long)field * gridDim.x + blockIdx.x] = t;
     }
+}
+
+// Single mode: the C-ABI carries the state as doubles; the handle stores floats.
+template <typename From, typename To>
+__global__ void __launch_bounds__(256) convert_state_kernel(const From* __restrict__ src, To* __restrict__ dst, long long n)
+{
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (long long)gridDim.x * blockDim.x)
+        dst[c] = (To)src[c];
 }
 
 // out[field] = sum over blocks, one thread per field.

@@ -13,17 +13,18 @@ namespace kh {
 
 // Primitive state of the (possibly ghost) cell at coordinates c[3], in the frame whose normal
 // is axis d: u = v_d, v = v_{d+1}, w = v_{d+2} (cyclic).  Counts floor hits only for cells the
-// caller owns (count = true).
-template <typename T>
-__device__ __forceinline__ Prim<T> load_prim(const double* __restrict__ U, const Grid& g, int ci, int cj, int ck,
-                                             int d, double gm1, int* hits)
+// caller owns (count = true).  S = float2_t, the type the conserved state is stored in (double; float in the
+// all-fp32 "Single" mode, where the recovery runs in fp32 as well).
+template <typename T, typename S = double>
+__device__ __forceinline__ Prim<T> load_prim(const S* __restrict__ U, const Grid& g, int ci, int cj, int ck,
+                                             int d, S gm1, int* hits)
 {
     int rx, ry, rz;
     const int si = g.active[0] ? bc_source(ci, g.n[0], g.bc[0], g.bc[1], rx) : (rx = VN_KEEP, 0);
     const int sj = g.active[1] ? bc_source(cj, g.n[1], g.bc[2], g.bc[3], ry) : (ry = VN_KEEP, 0);
     const int sk = g.active[2] ? bc_source(ck, g.n[2], g.bc[4], g.bc[5], rz) : (rz = VN_KEEP, 0);
     const long long c = cell_index(g, si, sj, sk);
-    double rho, p, vx, vy, vz;
+    S rho, p, vx, vy, vz;
     const int h = cons_to_prim(U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c], gm1, p, vx, vy,
                                vz, rho);
     if (hits) *hits += h;
@@ -33,7 +34,7 @@ __device__ __forceinline__ Prim<T> load_prim(const double* __restrict__ U, const
     Prim<T> W;
     W.r = T(rho);
     W.p = T(p);
-    const double vv[3] = {vx, vy, vz};
+    const S vv[3] = {vx, vy, vz};
     W.u = T(vv[d]);
     W.v = T(vv[(d + 1) % 3]);
     W.w = T(vv[(d + 2) % 3]);
@@ -42,11 +43,11 @@ __device__ __forceinline__ Prim<T> load_prim(const double* __restrict__ U, const
 
 // Flux through the low face (coordinate c_d - 1/2) of cell (ci,cj,ck) along axis d, returned in
 // conserved-field order (rho, m_x, m_y, m_z, eps).
-template <typename T>
-__device__ __noinline__ void face_flux_global(const double* __restrict__ U, const Grid& g, int ci, int cj, int ck,
+template <typename T, typename S = double>
+__device__ __noinline__ void face_flux_global(const S* __restrict__ U, const Grid& g, int ci, int cj, int ck,
                                               int d, T Fout[5])
 {
-    const double gm1 = g.gamma - 1.0;
+    const S gm1 = S(g.gamma - 1.0);
     const GasConst<T> gc(g.gamma, 0.0);
     int c[3] = {ci, cj, ck};
     Prim<T> W[4];
@@ -54,7 +55,7 @@ __device__ __noinline__ void face_flux_global(const double* __restrict__ U, cons
     for (int s = 0; s < 4; s++) {
         int cc[3] = {c[0], c[1], c[2]};
         cc[d] += s - 2;
-        W[s] = load_prim<T>(U, g, cc[0], cc[1], cc[2], d, gm1, nullptr);
+        W[s] = load_prim<T, S>(U, g, cc[0], cc[1], cc[2], d, gm1, nullptr);
     }
     Prim<T> L, R;
     // left state: cell c-1 plus its half slope; right state: cell c minus its half slope
@@ -79,8 +80,8 @@ __device__ __noinline__ void face_flux_global(const double* __restrict__ U, cons
 
 // One Heun stage.  STAGE 1: Uout = Uin + dt L(Uin).
 // STAGE 2: Uout = 1/2 U0 + 1/2 (Uin + dt L(Uin)) (Uout may alias U0), plus the CFL rate of Uout.
-template <typename T, int STAGE>
-__global__ void __launch_bounds__(128) stage_simple(const double* __restrict__ Uin, const double* U0, double* Uout,
+template <typename T, int STAGE, typename S = double>
+__global__ void __launch_bounds__(128) stage_simple(const S* __restrict__ Uin, const S* U0, S* Uout,
                                                     Grid g, Ctrl* ctrl)
 {
     __shared__ double red[32];
@@ -92,35 +93,35 @@ __global__ void __launch_bounds__(128) stage_simple(const double* __restrict__ U
         const int i = (int)(c % g.n[0]);
         const int j = (int)((c / g.n[0]) % g.n[1]);
         const int k = (int)(c / ((long long)g.n[0] * g.n[1]));
-        double dU[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        S dU[5] = {S(0), S(0), S(0), S(0), S(0)};   // float2_t accumulation
         for (int d = 0; d < 3; d++) {
             if (!g.active[d]) continue;
-            const double dtdx = dt * g.inv_dx[d];
+            const S dtdx = S(dt * g.inv_dx[d]);
             for (int side = 0; side < 2; side++) {
                 int cc[3] = {i, j, k};
                 cc[d] += side;
                 T F[5];
-                face_flux_global<T>(Uin, g, cc[0], cc[1], cc[2], d, F);
-                const double sgn = side ? -dtdx : dtdx;
+                face_flux_global<T, S>(Uin, g, cc[0], cc[1], cc[2], d, F);
+                const S sgn = side ? -dtdx : dtdx;
 #pragma unroll
-                for (int m = 0; m < 5; m++) dU[m] += sgn * (double)F[m];
+                for (int m = 0; m < 5; m++) dU[m] = fma_(sgn, (S)F[m], dU[m]);
             }
         }
         // floor statistics: count the primitive recovery of this thread's own cell once per stage
         {
-            double p, vx, vy, vz, rho;
+            S p, vx, vy, vz, rho;
             hits = cons_to_prim(Uin[c], Uin[g.N + c], Uin[2 * g.N + c], Uin[3 * g.N + c], Uin[4 * g.N + c],
-                                g.gamma - 1.0, p, vx, vy, vz, rho);
+                                S(g.gamma - 1.0), p, vx, vy, vz, rho);
         }
-        double Un[5];
+        S Un[5];
 #pragma unroll
         for (int m = 0; m < 5; m++) {
-            const double u = Uin[m * g.N + c] + dU[m];
-            Un[m] = (STAGE == 1) ? u : 0.5 * U0[m * g.N + c] + 0.5 * u;
+            const S u = add_(Uin[m * g.N + c], dU[m]);
+            Un[m] = (STAGE == 1) ? u : fma_(S(0.5), U0[m * g.N + c], mul_(S(0.5), u));
             Uout[m * g.N + c] = Un[m];
         }
         if (STAGE == 2) {
-            rate = (double)cfl_rate_from_cons<T>(Un, CflConst<T>(g));
+            rate = (double)cfl_rate_from_cons<T, S>(Un, CflConst<T>(g));
             if (!(rate == rate)) rate = __longlong_as_double(0x7ff0000000000000LL);
         }
     }

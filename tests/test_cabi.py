@@ -45,7 +45,8 @@ def test_bad_arguments_are_rejected():
     assert not L.kratos_hydro_create(2, 1, 1, 1.4, 0, bc)          # active axis with < 4 cells
     assert "4" in binding.last_error()
     assert not L.kratos_hydro_create(16, 1, 1, 1.0, 0, bc)         # gamma <= 1
-    assert not L.kratos_hydro_create(16, 1, 1, 1.4, 2, bc)         # unknown precision
+    assert not L.kratos_hydro_create(16, 1, 1, 1.4, 3, bc)         # unknown precision
+    assert not L.kratos_hydro_create(16, 1, 1, 1.4, 2 | (1 << 4), bc)   # all-fp32 state with the van Leer integrator
     bc_half = (ctypes.c_int * 6)(0, 1, 0, 0, 0, 0)
     assert not L.kratos_hydro_create(16, 1, 1, 1.4, 0, bc_half)    # periodic on one side only
     assert "periodic" in binding.last_error()

@@ -741,3 +741,74 @@ def test_strip_kernel_against_paired_kernel_and_conservation():
     assert (np.abs(T1 - T0) / np.maximum(np.maximum(np.abs(T0), A0), 1e-300)).max() <= 1e-13
     with pytest.raises(Exception):   # odd extents are refused, not silently served by another kernel
         binding.KratosHydro(37, 21, 1, 1.4, (P,) * 6, precision=MIXED, kernel=STRIP)
+
+
+# --------------------------------------------------------------------------- all-fp32 "Single" mode (Tables 1-2 "Single")
+from parity_utils import assert_parity_single  # noqa: E402
+
+SINGLE = binding.PREC_SINGLE
+CASES_SINGLE = [((45, 19, 23), (P, P, P, P, P, P)), ((64, 32, 10), (F, F, O, O, R, R)), ((96, 48, 12), (R, O, P, P, F, R)),
+                ((37, 21, 1), (P, P, P, P, P, P)), ((64, 48, 1), (R, R, O, F, P, P)), ((100, 38, 1), (P, P, F, R, P, P)),
+                ((50, 1, 1), (F, F, P, P, P, P)), ((1, 20, 22), (P, P, R, R, P, P))]
+
+
+def r32(U):
+    """The state as the Single mode stores it: rounded to fp32 (both sides start from this array)."""
+    return np.ascontiguousarray(U.astype(np.float32).astype(np.float64))
+
+
+@pytest.mark.parametrize("kernel", [binding.KERNEL_AUTO, SIMPLE])
+@pytest.mark.parametrize("shape,bc", CASES_SINGLE)
+def test_single_mode_parity(shape, bc, kernel):
+    """float2_t = float_t = float: state stored, updated and averaged in fp32.  Against the fp64 oracle within
+    parity_utils.tol_single (mixed-precision bound + 4 n 2^-24 for the fp32 storage, reading S16)."""
+    nx, ny, nz = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=nx + ny + nz, gamma=1.4, bc=bc)
+    U = r32(pr.U)
+    Uo = U.copy()
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=SINGLE, kernel=kernel)
+    h.set_state(U)
+    np.testing.assert_array_equal(h.get_state(), U)      # fp32-representable values cross the boundary unchanged
+    nsteps = 6
+    for _ in range(nsteps):
+        dt = oracle.cfl_dt(Uo, pr.gamma, 0.4)
+        oracle.step(Uo, pr.gamma, pr.bc, dt)
+        h.step(dt)
+    h.status()
+    Ug, hits = h.get_state(), h.floor_hits()
+    h.destroy()
+    assert hits == 0
+    assert np.array_equal(Ug, r32(Ug))                    # the state is fp32
+    assert_parity_single(Ug, Uo, pr.gamma, nsteps, what=str((shape, bc)))
+
+
+def test_single_mode_run_conservation_and_fixed_point():
+    """run() with the device-resident dt; totals conserved to fp32 rounding (PAPER.md:232-238 promises float2_t
+    accuracy, and float2_t is float here): within the storage bound, and visibly above the 1e-13 of the fp64 state;
+    a uniform state is still a bitwise fixed point."""
+    pr = inputs.turbulence_3d(64, seed=7, nsteps=20)
+    U = r32(pr.U)
+    Uo = U.copy()
+    oracle.run(Uo, pr.gamma, pr.bc, 0.4, 20)
+    h = binding.KratosHydro(64, 64, 64, pr.gamma, pr.bc, precision=SINGLE)
+    h.set_state(U)
+    T0 = h.totals()
+    np.testing.assert_allclose(T0, [math.fsum(U[m].ravel()) for m in range(5)], rtol=2e-16, atol=1e-9)
+    dt0 = h.cfl_dt(0.4)
+    assert dt0 == pytest.approx(oracle.cfl_dt(U, pr.gamma, 0.4), rel=1e-13)
+    h.run(0.4, 20)
+    T1, Ug = h.totals(), h.get_state()
+    h.destroy()
+    assert_parity_single(Ug, Uo, pr.gamma, 20)
+    A0 = np.array([math.fsum(np.abs(U[m]).ravel()) for m in range(5)])
+    drift = (np.abs(T1 - T0) / np.maximum(np.abs(T0), A0)).max()
+    assert drift <= 4 * 20 * 2.0 ** -24
+    U0 = r32(np.ascontiguousarray(inputs.prim_to_cons(np.full((12, 20, 40), 1.25), 0.75, 0.5, -1.0, 2.0, 1.5)))
+    h = binding.KratosHydro(40, 20, 12, 1.5, (P,) * 6, precision=SINGLE)
+    h.set_state(U0)
+    for _ in range(3):
+        h.step(1e-3)
+    np.testing.assert_array_equal(h.get_state(), U0)
+    h.destroy()
+    with pytest.raises(Exception):   # the van Leer integrator is not offered with an fp32 state
+        binding.KratosHydro(40, 20, 12, 1.5, (P,) * 6, precision=SINGLE, integrator=VL)
