@@ -35,6 +35,8 @@ UNIT = "cell-updates/s"
 BYTES_PER_CELL = {"stage1": 80.0, "stage2": 120.0}  # algorithmic HBM bytes per cell
 # van Leer, mixed precision: predictor 40 B read + 20 B written, corrector 20 + 40 read + 40 written
 BYTES_PER_CELL_VL = {"stage1": 60.0, "stage2": 100.0}
+# all-fp32 "Single" mode: the state is stored as floats, half the traffic of the Heun stages
+BYTES_PER_CELL_SINGLE = {"stage1": 40.0, "stage2": 60.0}
 
 
 def workload(name: str):
@@ -60,6 +62,9 @@ def workload(name: str):
 
 def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto", shape=(0, 0, 0)) -> str:
     """Name of the stage kernel the library launches for this block."""
+    if prec == 2:
+        tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0 and variant in ("auto", "tma")
+        return f"stage_tma<{stage},0,float>" if tma_ok else f"stage_simple<float,{stage},float>"
     if variant == "simple":
         return f"stage_simple<{'float' if prec == 0 else 'double'},{stage}>"
     tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0
@@ -198,14 +203,14 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     pr, wl_name = workload(args.workload)
-    prec = binding.PREC_MIXED if args.precision == "mixed" else binding.PREC_FP64
+    prec = {"mixed": binding.PREC_MIXED, "fp64": binding.PREC_FP64, "single": binding.PREC_SINGLE}[args.precision]
     nx, ny, nz = pr.shape
     ncell = pr.ncell
     stream = torch.cuda.Stream()
     variant = {"auto": binding.KERNEL_AUTO, "simple": binding.KERNEL_SIMPLE, "tiled": binding.KERNEL_TILED,
                "paired": binding.KERNEL_PAIRED, "tma": binding.KERNEL_TMA}[args.kernel]
     vanleer = args.integrator == "vanleer"
-    bpc = dict(BYTES_PER_CELL)
+    bpc = dict(BYTES_PER_CELL_SINGLE if prec == binding.PREC_SINGLE else BYTES_PER_CELL)
     if vanleer:
         bpc = dict(BYTES_PER_CELL_VL) if prec == binding.PREC_MIXED else {"stage1": 80.0, "stage2": 120.0}
     step_bytes = bpc["stage1"] + bpc["stage2"]
@@ -309,7 +314,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32 flux / f64 state" if prec == 0 else "f64", "data": "synthetic",
+        "vs_baseline": None, "dtype": {0: "f32 flux / f64 state", 1: "f64", 2: "f32"}[prec], "data": "synthetic",
         "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": args.precision,
                    "scheme": "PLM-minmod + HLLC + " + ("van Leer" if vanleer else "Heun"), "kernel": args.kernel, "cfl": pr.cfl, "parallelism": f"replicas x{world}",
                    "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
@@ -333,7 +338,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5")
-    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
+    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64", "single"],
+                    help="mixed: fp32 flux / fp64 state (the headline); fp64: all-fp64; single: all-fp32 (PAPER.md:240)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "tma"],

@@ -139,7 +139,8 @@ void collect_timing(kratos_hydro* h)
 int auto_variant(const kratos_hydro* h)
 {
     if (h->integ == 1) return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;  // van Leer
-    if (h->prec == KRATOS_PREC_SINGLE) return KRATOS_KERNEL_SIMPLE;   // all-fp32 state: the general kernel
+    if (h->prec == KRATOS_PREC_SINGLE)   // all-fp32 state: the TMA kernel on float boxes, else the general kernel
+        return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
     if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
@@ -193,7 +194,8 @@ int launch_stage_single(kratos_hydro* h, int stage)
     LaunchTimer lt(h, stage == 1 ? SLOT_STAGE1 : SLOT_STAGE2);
     const int threads = 128;
     const long long blocks = (g.N + threads - 1) / threads;
-    if (stage == 1) stage_simple<float, 1, float><<<(unsigned)blocks, threads, 0, h->stream>>>(A, A, B, g, h->ctrl);
+    if (h->variant == KRATOS_KERNEL_TMA) tma::launch_stage_single(stage, *h->maps, g, h->ctrl, pick_zchunk(h), h->stream);
+    else if (stage == 1) stage_simple<float, 1, float><<<(unsigned)blocks, threads, 0, h->stream>>>(A, A, B, g, h->ctrl);
     else            stage_simple<float, 2, float><<<(unsigned)blocks, threads, 0, h->stream>>>(B, A, const_cast<float*>(A), g, h->ctrl);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "stage %d launch: %s", stage, cudaGetErrorString(e));
@@ -399,6 +401,10 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     pr::configure();
     tma::configure();
     strip::configure();
+    if (prec == KRATOS_PREC_SINGLE && tma::supported(g)) {
+        h->maps = new (std::nothrow) tma::StageMaps;
+        if (h->maps) tma::build_maps_single(h->maps, reinterpret_cast<const float*>(h->U0), reinterpret_cast<const float*>(h->U1), g);
+    }
     if (prec == KRATOS_PREC_MIXED && tma::supported(g)) {
         h->maps = new (std::nothrow) tma::StageMaps;
         if (h->maps && integ == 0) tma::build_maps(h->maps, h->U0, h->U1, g);

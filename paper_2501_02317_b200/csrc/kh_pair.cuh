@@ -188,6 +188,21 @@ __device__ __forceinline__ int recover(double rho, double mx, double my, double 
     return (int)lo_r + (int)lo_p;
 }
 
+// All-fp32 "Single" mode (float2_t = float_t = float): the recovery on an fp32 state, in fp32
+// (kh::cons_to_prim(float...): explicitly rounded, 1/rho by MUFU.RCP); no reference pressure (pref = 0).
+__device__ __forceinline__ int recover(float rho, float mx, float my, float mz, float e, float gm1, float pref, int rx, int ry,
+                                       int rz, float W[5])
+{
+    float p, vx, vy, vz, r;
+    const int hits = cons_to_prim(rho, mx, my, mz, e, gm1, p, vx, vy, vz, r);
+    W[0] = r;
+    W[1] = __fadd_rn(p, -pref);
+    W[2] = apply_vn_rule(vx, rx);
+    W[3] = apply_vn_rule(vy, ry);
+    W[4] = apply_vn_rule(vz, rz);
+    return hits;
+}
+
 template <int STAGE>
 struct Smem {
     double2 raw[NSLOT][5][PRP][PTX];                          // fp64 state of (row 2w, row 2w+1) at a column

@@ -24,6 +24,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "kh_pair.cuh"
 
 namespace kh {
@@ -78,7 +80,8 @@ constexpr int OWN_BYTES = 5 * PTY * PTX * 8;    // one tile box
 constexpr int ROW_BYTES = 5 * 2 * PTX * 8;      // one halo row pair
 constexpr int COL_BYTES = 5 * PTY * 2 * 8;      // one halo column pair
 
-template <int STAGE, int MODE = 0>
+// ST = float2_t, the type the conserved state is stored in: double, or float in the all-fp32 "Single" mode (MODE 0 only).
+template <int STAGE, int MODE = 0, typename ST = double>
 struct Smem {
     static constexpr int NSLOT = Cfg<STAGE>::NSLOT;
     static constexpr int NHALO = Cfg<STAGE>::NHALO;
@@ -86,8 +89,8 @@ struct Smem {
     // refill of a slot then never waits for the store that is still reading the previous plane)
     static constexpr int NU0 = (STAGE == 2) ? ((MODE == 2) ? 3 : 2) : 1;
     // planes in flight: fp64 conserved state, or (van Leer corrector) float_t primitives = half the bytes
-    alignas(128) double raw[NSLOT][5][(MODE == 2) ? PTY / 2 : PTY][PTX];
-    alignas(128) double u0[NU0][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
+    alignas(128) ST raw[NSLOT][5][(MODE == 2) ? PTY / 2 : PTY][PTX];
+    alignas(128) ST u0[NU0][(STAGE == 2) ? 5 : 1][(STAGE == 2) ? PTY : 1][PTX];
     alignas(128) double hrow[NHALO][2][5][2][PTX];            // halo rows: [lo/hi][field][box row][column]
     alignas(128) double hcol[NHALO][2][5][PTY][2];            // halo columns: [lo/hi][field][row][box column]
     f2 Wt[5][PRP + 2][PTX + 4];                               // primitives of one plane, row pairs -1..PRP, columns -2..PTX+1
@@ -311,13 +314,17 @@ __device__ __forceinline__ void plm_m(f2 qm, f2 q, f2 qp, f2& qL, f2& qR)
 // primitives W^{n+1/2} = prim(U + dt/2 L_1(U)) (a float box written over the consumed raw plane and stored by TMA).
 // MODE 2 (with STAGE 2): its corrector U^{n+1} = U^n + dt L_2(W^{n+1/2}): the plane ring and the halo boxes carry the
 // float_t primitives (no recovery, no fp64 chain), U^n arrives through the U0 ring, is updated in place there and stored.
-template <int STAGE, int MODE = 0>
+template <int STAGE, int MODE = 0, typename ST = double>
 __global__ void __launch_bounds__(NTHREADS, BLOCKS_PER_SM)
 stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
     static_assert(MODE == 0 || (MODE == 1 && STAGE == 1) || (MODE == 2 && STAGE == 2),
                   "the van Leer predictor has the data flow of stage 1, the corrector that of stage 2");
-    using S = Smem<STAGE, MODE>;
+    constexpr bool SGL = sizeof(ST) == 4;          // all-fp32 "Single" mode: fp32 state, update and boxes
+    static_assert(!SGL || MODE == 0, "the fp32 state comes with the Heun integrator only");
+    constexpr bool FBOX = SGL || MODE == 2;        // the stage input arrives as float boxes
+    using S = Smem<STAGE, MODE, ST>;
+    using ST2 = typename std::conditional<SGL, float2, double2>::type;
     constexpr int NU0 = S::NU0;
     constexpr int NSLOT = S::NSLOT;
     constexpr int NHALO = S::NHALO;
@@ -326,7 +333,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
     const double dt = (MODE == 1) ? 0.5 * ctrl->dt : ctrl->dt;
     if (!(dt > 0.0)) return;  // a step clipped to zero length (run_until past t_end) does nothing
-    const double pref_d = ctrl->p_ref;
+    const double pref_d = SGL ? 0.0 : ctrl->p_ref;   // (fp32 state: the deviation from a reference pressure gains nothing)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const int i0 = blockIdx.x * PTX, j0 = blockIdx.y * PTY;
@@ -334,7 +341,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
     const int kend = min(kbeg + zchunk, nz);
     const int kfirst = kbeg - 1;  // priming iteration: builds the tile of plane kbeg
     const int pbase = kbeg - 2;   // first plane of the raw ring: plane p sits in slot (p - pbase) % NSLOT
-    const double gm1 = g.gamma - 1.0;
+    const ST gm1 = ST(g.gamma - 1.0);
+    const ST pref_s = ST(pref_d);
     Gas gas;
     gas.gamma = (float)g.gamma;
     gas.g1 = (float)((g.gamma + 1.0) / (2.0 * g.gamma));
@@ -356,20 +364,20 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         // ================================ main warps: cells (i, ja), (i, ja+1) ========================
         asm volatile("setmaxnreg.inc.sync.aligned.u32 " KH_TMA_STR(KH_TMA_MAIN_REGS) ";");
         const int w = warp;
-        constexpr int RAWF = PTY * PTX, RAWS = 5 * RAWF;              // double strides of raw / u0: field, slot
+        constexpr int RAWF = PTY * PTX, RAWS = 5 * RAWF;              // element strides of raw / u0: field, slot
         constexpr int WTF = (PRP + 2) * (PTX + 4);                    // f2 field stride of Wt
         constexpr int QXF = PRP * (PTX + 1);                          // f2 field stride of QLx, double2 of Fx
         constexpr int QYF = (PRP + 1) * PTX;                          // field stride of QLy (float) and Fy (double)
-        double* const raw0 = (MODE == 2) ? &sm.raw[0][0][0][0]        // (float planes: addressed in convert)
-                                         : &sm.raw[0][0][2 * w][lane]; // row 2w; row 2w+1 is + PTX
-        const double* const u00 = &sm.u0[0][0][(STAGE == 2) ? 2 * w : 0][lane];
+        ST* const raw0 = (MODE == 2) ? &sm.raw[0][0][0][0]            // (float planes: addressed in convert)
+                                     : &sm.raw[0][0][2 * w][lane];     // row 2w; row 2w+1 is + PTX
+        const ST* const u00 = &sm.u0[0][0][(STAGE == 2) ? 2 * w : 0][lane];
         f2* const wt = &sm.Wt[0][w + 1][lane + 2];
         f2* const qlx = &sm.QLx[0][w][lane];      // left state of the own low x face; own high face is + 1
         float* const qly = &sm.QLy[0][w][lane];   // left state of the pair's low y face; the pair's high face is + PTX
         f2* const fxs = &sm.Fx[0][w][lane];
         float* const fys = &sm.Fy[0][w][lane];
 
-        const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1], dtdz = dt * g.inv_dx[2];
+        const ST dtdx = ST(dt * g.inv_dx[0]), dtdy = ST(dt * g.inv_dx[1]), dtdz = ST(dt * g.inv_dx[2]);
         const CflConst<float> cc(g);
 
         // conversion of plane kk (ring index q = kk - pbase): wait for its box, recover the pair's primitives
@@ -386,13 +394,13 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 W[4] = mk(apply_vn_rule(W[4].x, rz), apply_vn_rule(W[4].y, rz));
                 return;
             }
-            const double* s = raw0 + slot * RAWS;
-            double ua[5], ub[5];
+            const ST* s = raw0 + slot * RAWS;
+            ST ua[5], ub[5];
 #pragma unroll
             for (int f = 0; f < 5; f++) { ua[f] = s[f * RAWF]; ub[f] = s[f * RAWF + PTX]; }
             float Wa[5], Wb[5];
-            const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, VN_KEEP, VN_KEEP, rz, Wa);
-            const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, VN_KEEP, VN_KEEP, rz, Wb);
+            const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_s, VN_KEEP, VN_KEEP, rz, Wa);
+            const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_s, VN_KEEP, VN_KEEP, rz, Wb);
             if (count) hits += ha + hb;
 #pragma unroll
             for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
@@ -400,7 +408,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
         // ---- prologue: planes kbeg-2 .. kbeg+1 (ring slots 0 .. 3, first fill: parity 0) ----
         f2 Wa[5], Wb[5], Wn[5], QLz[5];   // W(k), W(k+1), W(k+2), left state of z face k+1/2
-        double2 Fzlo[5];           // dt/dz * flux through z face k-1/2
+        ST2 Fzlo[5];               // dt/dz * flux through z face k-1/2
         {
             f2 Wm[5];
             convert(kbeg - 2, 0, 0u, Wm, false);
@@ -411,7 +419,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             for (int f = 0; f < 5; f++) {
                 f2 qR;
                 plm_m<MODE>(Wm[f], Wa[f], Wb[f], QLz[f], qR);
-                Fzlo[f] = make_double2(0.0, 0.0);
+                Fzlo[f].x = Fzlo[f].y = ST(0);
             }
         }
         // ring positions of the planes k+3 (converted) and k (updated) at the first iteration k = kfirst
@@ -421,9 +429,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 
         f2 QRx[5], QRy[5];
         float QLyo[5];  // left state of the face between the pair's two cells
-        double2 dU[5];
+        ST2 dU[5];
 #pragma unroll
-        for (int f = 0; f < 5; f++) { QRx[f] = QRy[f] = mk(0.f, 0.f); QLyo[f] = 0.f; dU[f] = make_double2(0.0, 0.0); }
+        for (int f = 0; f < 5; f++) { QRx[f] = QRy[f] = mk(0.f, 0.f); QLyo[f] = 0.f; dU[f].x = dU[f].y = ST(0); }
 
 #pragma unroll UNROLL
         for (int k = kfirst; k < kend; k++) {
@@ -433,7 +441,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             // The z, x and y Riemann problems of the pair are independent: they are solved in lock step
             // (hllc2n).  In the priming iteration the x / y inputs are not valid yet; those results are
             // computed all the same (one basic block) and never used.
-            double2 Fzhi[5];
+            ST2 Fzhi[5];
             f2 Wn2[5];
             {
                 f2 L[3][5], R[3][5], Fn[3][5], F[5];
@@ -462,24 +470,23 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 from_normal<2>(Fn[0], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    Fzhi[f] = make_double2(__dmul_rn(dtdz, (double)F[f].x), __dmul_rn(dtdz, (double)F[f].y));
-                    dU[f] = make_double2(__dadd_rn(Fzlo[f].x, -Fzhi[f].x), __dadd_rn(Fzlo[f].y, -Fzhi[f].y));
+                    Fzhi[f].x = mul_(dtdz, (ST)F[f].x); Fzhi[f].y = mul_(dtdz, (ST)F[f].y);
+                    dU[f].x = sub_(Fzlo[f].x, Fzhi[f].x); dU[f].y = sub_(Fzlo[f].y, Fzhi[f].y);
                 }
                 from_normal<0>(Fn[1], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double2 fd = make_double2((double)F[f].x, (double)F[f].y);
                     fxs[f * QXF] = F[f];
-                    dU[f].x = __fma_rn(dtdx, fd.x, dU[f].x);
-                    dU[f].y = __fma_rn(dtdx, fd.y, dU[f].y);
+                    dU[f].x = fma_(dtdx, (ST)F[f].x, dU[f].x);
+                    dU[f].y = fma_(dtdx, (ST)F[f].y, dU[f].y);
                 }
                 from_normal<1>(Fn[2], F);
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
-                    const double flo = (double)F[f].x, fin = (double)F[f].y;
+                    const ST flo = (ST)F[f].x, fin = (ST)F[f].y;
                     fys[f * QYF] = F[f].x;
-                    dU[f].x = __fma_rn(dtdy, __dadd_rn(flo, -fin), dU[f].x);
-                    dU[f].y = __fma_rn(dtdy, fin, dU[f].y);
+                    dU[f].x = fma_(dtdy, sub_(flo, fin), dU[f].x);
+                    dU[f].y = fma_(dtdy, fin, dU[f].y);
                 }
             }
             if (k + 1 < kend) {
@@ -488,11 +495,11 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             }
             // The thread's own fp64 data for the update (nobody else touches these entries) are fetched BEFORE the barrier:
             // their latency hides behind the barrier wait and they stay out of the load burst that follows it.
-            double* const su = raw0 + s_upd * RAWS;
+            ST* const su = raw0 + s_upd * RAWS;
             const int m0 = max(k - kbeg, 0);
-            const double* const s0 = u00 + (m0 % NU0) * RAWS;
+            const ST* const s0 = u00 + (m0 % NU0) * RAWS;
             if (STAGE == 2 && live) mbar_wait_parity(&sm.full_u0[m0 % NU0], (unsigned)(m0 / NU0) & 1u);
-            double ua[5], ub[5], va[5], vb[5];
+            ST ua[5], ub[5], va[5], vb[5];
 #pragma unroll
             for (int f = 0; f < 5; f++) {
                 if (MODE != 2) {
@@ -530,12 +537,12 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
                     // the state the flux differences are added to: the stage input (Heun), U^n (van Leer corrector)
-                    const double ba = (MODE == 2) ? va[f] : ua[f], bb = (MODE == 2) ? vb[f] : ub[f];
-                    double xa = __dadd_rn(ba, __fma_rn(-dtdx, (double)fxh[f].x, dU[f].x));
-                    double xb = __dadd_rn(bb, __fma_rn(-dtdy, (double)fyh[f], __fma_rn(-dtdx, (double)fxh[f].y, dU[f].y)));
+                    const ST ba = (MODE == 2) ? va[f] : ua[f], bb = (MODE == 2) ? vb[f] : ub[f];
+                    ST xa = add_(ba, fma_(-dtdx, (ST)fxh[f].x, dU[f].x));
+                    ST xb = add_(bb, fma_(-dtdy, (ST)fyh[f], fma_(-dtdx, (ST)fxh[f].y, dU[f].y)));
                     if (STAGE == 2 && MODE == 0) {
-                        xa = __fma_rn(0.5, va[f], __dmul_rn(0.5, xa));
-                        xb = __fma_rn(0.5, vb[f], __dmul_rn(0.5, xb));
+                        xa = fma_(ST(0.5), va[f], mul_(ST(0.5), xa));
+                        xb = fma_(ST(0.5), vb[f], mul_(ST(0.5), xb));
                     }
                     ua[f] = xa;
                     ub[f] = xb;
@@ -575,8 +582,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     // W^{n+1/2} as float_t primitives (actual pressure: offset 0), written as a float box [5][PTY][PTX]
                     // over the head of the raw plane just consumed (every thread read its entries before barrier 2)
                     float Wpa[5], Wpb[5];
-                    const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, 0.0, VN_KEEP, VN_KEEP, VN_KEEP, Wpa);
-                    const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, 0.0, VN_KEEP, VN_KEEP, VN_KEEP, Wpb);
+                    const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, ST(0), VN_KEEP, VN_KEEP, VN_KEEP, Wpa);
+                    const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, ST(0), VN_KEEP, VN_KEEP, VN_KEEP, Wpb);
                     if (live) hits += ha + hb;
                     float* const sf = reinterpret_cast<float*>(raw0 + s_upd * RAWS - (2 * w * PTX + lane)) + (2 * w * PTX + lane);
 #pragma unroll
@@ -592,7 +599,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                         su[f * RAWF + PTX] = ub[f];
                     }
                     if (MODE == 2 && live) {  // U^{n+1} over U^n in the U0 ring: the producer ships that box
-                        double* const sv = const_cast<double*>(s0);
+                        ST* const sv = const_cast<ST*>(s0);
                         sv[f * RAWF] = ua[f];
                         sv[f * RAWF + PTX] = ub[f];
                     }
@@ -687,19 +694,27 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             if (k + 1 < kend) {
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = h0 + hs * HSLOT;
-                if (MODE == 2) {  // float primitives: [side][field][box row][column], 1280 bytes per side
+                if (FBOX) {  // float boxes: [side][field][box row][column], 1280 bytes per side
                     const float* sf = reinterpret_cast<const float*>(s) + (top ? 5 * 2 * PTX : 0) + lane;
                     const float pref_f = (float)pref_d;
 #pragma unroll
                     for (int f = 0; f < 5; f++) { W0[f] = sf[f * 2 * PTX + hsd.idx0 * PTX]; W1[f] = sf[f * 2 * PTX + hsd.idx1 * PTX]; }
-                    W0[1] = pdev(W0[1], pref_f); W1[1] = pdev(W1[1], pref_f);
-                    W0[3] = apply_vn_rule(W0[3], ry);  W1[3] = apply_vn_rule(W1[3], ry);
+                    if (SGL) {  // conserved fp32 state
+                        float c0[5], c1[5];
+#pragma unroll
+                        for (int f = 0; f < 5; f++) { c0[f] = W0[f]; c1[f] = W1[f]; }
+                        (void)recover(c0[0], c0[1], c0[2], c0[3], c0[4], (float)gm1, pref_f, VN_KEEP, ry, VN_KEEP, W0);
+                        (void)recover(c1[0], c1[1], c1[2], c1[3], c1[4], (float)gm1, pref_f, VN_KEEP, ry, VN_KEEP, W1);
+                    } else {    // float_t primitives of the van Leer predictor
+                        W0[1] = pdev(W0[1], pref_f); W1[1] = pdev(W1[1], pref_f);
+                        W0[3] = apply_vn_rule(W0[3], ry);  W1[3] = apply_vn_rule(W1[3], ry);
+                    }
                 } else {
                 double u0[5], u1[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) { u0[f] = s[off0 + f * HF]; u1[f] = s[off1 + f * HF]; }
-                (void)recover(u0[0], u0[1], u0[2], u0[3], u0[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W0);
-                (void)recover(u1[0], u1[1], u1[2], u1[3], u1[4], gm1, pref_d, VN_KEEP, ry, VN_KEEP, W1);
+                (void)recover(u0[0], u0[1], u0[2], u0[3], u0[4], (double)gm1, pref_d, VN_KEEP, ry, VN_KEEP, W0);
+                (void)recover(u1[0], u1[1], u1[2], u1[3], u1[4], (double)gm1, pref_d, VN_KEEP, ry, VN_KEEP, W1);
                 }
 #pragma unroll
                 for (int f = 0; f < 5; f++) wown[f * WTF] = mk(W0[f], W1[f]);
@@ -713,7 +728,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         const int cid = lane & 3, rp = min(lane >> 2, PRP - 1);     // column id, row pair
         const bool xact = (lane >> 2) < PRP;                        // (a tile of 8 rows keeps half the lanes busy)
         const int col = (cid < 2) ? cid - 2 : PTX + cid - 2;
-        constexpr int XW = (MODE == 2) ? 4 : 2;   // width of the halo column boxes (16 bytes: 2 doubles or 4 floats)
+        constexpr int XW = FBOX ? 4 : 2;   // width of the halo column boxes (16 bytes: 2 doubles or 4 floats)
         const HaloSide side = (cid < 2) ? halo_side(i0 - 2, nx, g.bc[0], g.bc[1], XW) : halo_side(i0 + PTX, nx, g.bc[0], g.bc[1], XW);
         const int bidx = (cid & 1) ? side.idx1 : side.idx0;
         const int rx = side.rule;
@@ -751,20 +766,28 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 mbar_wait_parity(&sm.full_halo[hs], hpar);
                 const double* s = c0 + hs * CSLOT;
                 float Wa[5], Wb[5];
-                if (MODE == 2) {  // float primitives: [side][field][row][box column], 4 columns per box, 1280 bytes per side
+                if (FBOX) {  // float boxes: [side][field][row][box column], 4 columns per box, 1280 bytes per side
                     const float* sf = reinterpret_cast<const float*>(&sm.hcol[0][0][0][0][0] + hs * CSLOT) +
                                       (cid >> 1) * (5 * PTY * 4) + (2 * rp) * 4 + bidx;
                     const float pref_f = (float)pref_d;
 #pragma unroll
                     for (int f = 0; f < 5; f++) { Wa[f] = sf[f * PTY * 4]; Wb[f] = sf[f * PTY * 4 + 4]; }
-                    Wa[1] = pdev(Wa[1], pref_f); Wb[1] = pdev(Wb[1], pref_f);
-                    Wa[2] = apply_vn_rule(Wa[2], rx);  Wb[2] = apply_vn_rule(Wb[2], rx);
+                    if (SGL) {  // conserved fp32 state
+                        float ca[5], cb[5];
+#pragma unroll
+                        for (int f = 0; f < 5; f++) { ca[f] = Wa[f]; cb[f] = Wb[f]; }
+                        (void)recover(ca[0], ca[1], ca[2], ca[3], ca[4], (float)gm1, pref_f, rx, VN_KEEP, VN_KEEP, Wa);
+                        (void)recover(cb[0], cb[1], cb[2], cb[3], cb[4], (float)gm1, pref_f, rx, VN_KEEP, VN_KEEP, Wb);
+                    } else {    // float_t primitives of the van Leer predictor
+                        Wa[1] = pdev(Wa[1], pref_f); Wb[1] = pdev(Wb[1], pref_f);
+                        Wa[2] = apply_vn_rule(Wa[2], rx);  Wb[2] = apply_vn_rule(Wb[2], rx);
+                    }
                 } else {
                 double ua[5], ub[5];
 #pragma unroll
                 for (int f = 0; f < 5; f++) { ua[f] = s[f * CF]; ub[f] = s[f * CF + 2]; }
-                (void)recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wa);
-                (void)recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wb);
+                (void)recover(ua[0], ua[1], ua[2], ua[3], ua[4], (double)gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wa);
+                (void)recover(ub[0], ub[1], ub[2], ub[3], ub[4], (double)gm1, pref_d, rx, VN_KEEP, VN_KEEP, Wb);
                 }
 #pragma unroll
                 for (int f = 0; f < 5; f++) {
@@ -780,9 +803,10 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         // ================================ producer warp: all global traffic, by TMA =====================
         const HaloSide ylo = halo_side(j0 - 2, ny, g.bc[2], g.bc[3]);
         const HaloSide yhi = halo_side(j0 + PTY, ny, g.bc[2], g.bc[3]);
-        constexpr int XW = (MODE == 2) ? 4 : 2;                        // halo column boxes: 2 doubles or 4 floats wide
-        constexpr unsigned RAW_TX = (MODE == 2) ? OWN_BYTES / 2 : OWN_BYTES;   // float primitives are half the bytes
-        constexpr unsigned HALO_TX = (MODE == 2) ? 4 * 1280 : 2 * ROW_BYTES + 2 * COL_BYTES;
+        constexpr int XW = FBOX ? 4 : 2;                               // halo column boxes: 2 doubles or 4 floats wide
+        constexpr unsigned RAW_TX = FBOX ? OWN_BYTES / 2 : OWN_BYTES;  // float boxes are half the bytes
+        constexpr unsigned HALO_TX = FBOX ? 4 * 1280 : 2 * ROW_BYTES + 2 * COL_BYTES;
+        constexpr unsigned U0_TX = SGL ? OWN_BYTES / 2 : OWN_BYTES;
         const HaloSide xlo = halo_side(i0 - 2, nx, g.bc[0], g.bc[1], XW);
         const HaloSide xhi = halo_side(i0 + PTX, nx, g.bc[0], g.bc[1], XW);
         const int plast = kend + 2;  // planes up to kend+1 feed the z stencil; the main warps convert one plane further
@@ -797,9 +821,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             unsigned long long* bar = &sm.full_halo[slot];
             mbar_expect_tx(bar, HALO_TX);
             // second side of each pair: right behind the first one (float boxes are 1280 bytes each)
-            char* const r1 = (MODE == 2) ? reinterpret_cast<char*>(&sm.hrow[slot][0][0][0][0]) + 1280
+            char* const r1 = FBOX ? reinterpret_cast<char*>(&sm.hrow[slot][0][0][0][0]) + 1280
                                          : reinterpret_cast<char*>(&sm.hrow[slot][1][0][0][0]);
-            char* const c1 = (MODE == 2) ? reinterpret_cast<char*>(&sm.hcol[slot][0][0][0][0]) + 1280
+            char* const c1 = FBOX ? reinterpret_cast<char*>(&sm.hcol[slot][0][0][0][0]) + 1280
                                          : reinterpret_cast<char*>(&sm.hcol[slot][1][0][0][0]);
             tma_load4(&sm.hrow[slot][0][0][0][0], &maps.in_rows, i0, ylo.start, p, 0, bar);
             tma_load4(r1, &maps.in_rows, i0, yhi.start, p, 0, bar);
@@ -831,7 +855,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                     const int m = (k + 1 - kbeg) % NU0;
                     // this slot held plane k-2, whose store was committed one group before the one just issued
                     if (stored) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-                    mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
+                    mbar_expect_tx(&sm.full_u0[m], U0_TX);
                     tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
                 }
             }
@@ -844,7 +868,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
                 if (STAGE == 2 && k + 1 < kend) {
                     const int m = (k + 1 - kbeg) % NU0;
-                    mbar_expect_tx(&sm.full_u0[m], OWN_BYTES);
+                    mbar_expect_tx(&sm.full_u0[m], U0_TX);
                     tma_load4(&sm.u0[m][0][0][0], &maps.u0_own, i0, j0, k + 1, 0, &sm.full_u0[m]);
                 }
             }
@@ -970,6 +994,28 @@ inline void build_maps_vl(StageMaps* sm, const double* A, const float* Wh, const
     sm->ok = true;
 }
 
+// all-fp32 "Single" mode: both state arrays hold floats; stage 1 reads A writes B, stage 2 reads B, averages with and
+// writes A.  Halo column boxes are 4 floats (16 bytes) wide.
+inline void build_maps_single(StageMaps* sm, const float* A, const float* B, const Grid& g)
+{
+    sm->ok = false;
+    if (!supported(g) || (g.N * 4) % 16 != 0) return;
+    CUtensorMap a_own, a_rows, a_cols, b_own, b_rows, b_cols;
+    if (!make_map_f32(&a_own, A, g) || !make_map_f32(&a_rows, A, g, PTX, 2) || !make_map_f32(&a_cols, A, g, 4, PTY) ||
+        !make_map_f32(&b_own, B, g) || !make_map_f32(&b_rows, B, g, PTX, 2) || !make_map_f32(&b_cols, B, g, 4, PTY))
+        return;
+    sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = b_own;
+    sm->s2.in_own = b_own; sm->s2.in_rows = b_rows; sm->s2.in_cols = b_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
+    sm->ok = true;
+}
+
+inline void launch_stage_single(int stage, const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
+{
+    dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
+    if (stage == 1) stage_tma<1, 0, float><<<grid, NTHREADS, sizeof(Smem<1, 0, float>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
+    else            stage_tma<2, 0, float><<<grid, NTHREADS, sizeof(Smem<2, 0, float>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
+}
+
 inline void launch_vl_correct(const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
 {
     dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
@@ -1005,6 +1051,10 @@ inline void configure()
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_tma<1, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1, 0, float>) + 128);
+    cudaFuncSetAttribute(stage_tma<2, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2, 0, float>) + 128);
+    cudaFuncSetAttribute(stage_tma<1, 0, float>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_tma<2, 0, float>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
 }
 
 inline void launch_stage(int stage, const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
