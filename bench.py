@@ -60,19 +60,23 @@ def workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
-def kernel_name(prec: int, stage: int, ndim: int, variant: str = "auto", shape=(0, 0, 0)) -> str:
-    """Name of the stage kernel the library launches for this block."""
-    if prec == 2:
-        tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0 and variant in ("auto", "tma")
-        return f"stage_tma<{stage},0,float>" if tma_ok else f"stage_simple<float,{stage},float>"
-    if variant == "simple":
-        return f"stage_simple<{'float' if prec == 0 else 'double'},{stage}>"
-    tma_ok = ndim == 3 and shape[0] % 32 == 0 and shape[1] % 16 == 0
-    if prec == 0 and (variant == "tma" or (variant == "auto" and tma_ok)):
-        return f"stage_tma<{stage}>"
-    if prec == 0 and variant in ("auto", "paired"):
+def kernel_name(variant: int, prec: int, stage: int, ndim: int, vanleer: bool = False) -> str:
+    """Name of the stage kernel the library launches, from the variant the handle resolved."""
+    from paper_2501_02317_b200 import binding as b
+    ft = {0: "float", 1: "double", 2: "float"}[prec]
+    if vanleer:
+        if variant == b.KERNEL_TMA:
+            return "stage_tma<1,1>" if stage == 1 else "stage_tma<2,2>"
+        return ("vl::predict<%s>" if stage == 1 else "vl::correct<%s>") % ft
+    if variant == b.KERNEL_TMA:
+        return f"stage_tma<{stage},0,float>" if prec == 2 else f"stage_tma<{stage}>"
+    if variant == b.KERNEL_STRIP:
+        return f"stage_strip<{stage}>"
+    if variant == b.KERNEL_PAIRED:
         return f"stage_pair<{stage},{ndim}>"
-    return f"stage_tiled<{'float' if prec == 0 else 'double'},{stage},{ndim}>"
+    if variant == b.KERNEL_TILED:
+        return f"stage_tiled<{ft},{stage},{ndim}>"
+    return f"stage_simple<{ft},{stage},float>" if prec == 2 else f"stage_simple<{ft},{stage}>"
 
 
 def measured_peak():
@@ -218,6 +222,7 @@ def run_ours(args):
                             integrator=binding.INTEGRATOR_VANLEER if vanleer else binding.INTEGRATOR_HEUN)
     if args.zchunk > 0:
         h.set_zchunk(args.zchunk)
+    resolved = h.get_kernel()
     host = torch.from_numpy(pr.U).pin_memory()            # pinned host copy (e2e leg)
     with torch.cuda.stream(stream):
         dev = host.to("cuda", non_blocking=True)
@@ -289,11 +294,7 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
-        kname = kernel_name(prec, int(dom[-1]), 3 if nz > 1 else 2, args.kernel, (nx, ny, nz))
-        if vanleer:
-            kname = ("vl::predict<%s>" if dom == "stage1" else "vl::correct<%s>") % ("float" if prec == 0 else "double")
-            if prec == 0 and nz > 1 and nx % 32 == 0 and ny % 16 == 0 and args.kernel in ("auto", "tma"):
-                kname = "stage_tma<1,1>" if dom == "stage1" else "stage_tma<2,2>"
+        kname = kernel_name(resolved, prec, int(dom[-1]), 3 if nz > 1 else (2 if ny > 1 else 1), vanleer)
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                     "unit": "GB/s", "frac": kern[dom]["frac"],
                     "traffic": ncu_traffic(args.workload, args.precision, kname),

@@ -113,6 +113,9 @@ KRATOS_API int kratos_hydro_set_stream(kratos_hydro_t *h, void *cuda_stream);
  * support this block's active axes. */
 KRATOS_API int kratos_hydro_set_kernel(kratos_hydro_t *h, int variant);
 
+/* The kernel variant (KRATOS_KERNEL_*, never AUTO) that step / run launch for this handle.  variant: host. */
+KRATOS_API int kratos_hydro_get_kernel(kratos_hydro_t *h, int *variant);
+
 /* z-extent of the slab one thread block of the marching 3D kernels works through; for the 2D strip kernel the number
  * of rows (rounded up to even) one warp marches through (0 = automatic). */
 KRATOS_API int kratos_hydro_set_zchunk(kratos_hydro_t *h, int planes);

@@ -25,7 +25,7 @@ OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
 # every symbol include/kratos_hydro.h declares
 SYMBOLS = [
     "kratos_hydro_create", "kratos_hydro_destroy", "kratos_hydro_set_spacing", "kratos_hydro_set_stream",
-    "kratos_hydro_set_kernel", "kratos_hydro_set_zchunk", "kratos_hydro_set_state", "kratos_hydro_get_state",
+    "kratos_hydro_set_kernel", "kratos_hydro_get_kernel", "kratos_hydro_set_zchunk", "kratos_hydro_set_state", "kratos_hydro_get_state",
     "kratos_hydro_cfl_dt", "kratos_hydro_step", "kratos_hydro_run", "kratos_hydro_run_until",
     "kratos_hydro_totals", "kratos_hydro_floor_hits", "kratos_hydro_status", "kratos_hydro_launch_count",
     "kratos_hydro_set_profiling", "kratos_hydro_get_timing", "kratos_hydro_last_error", "kratos_hydro_version",
@@ -65,6 +65,8 @@ def load() -> ctypes.CDLL:
     L.kratos_hydro_set_stream.argtypes = [vp, vp]
     L.kratos_hydro_set_kernel.restype = i
     L.kratos_hydro_set_kernel.argtypes = [vp, i]
+    L.kratos_hydro_get_kernel.restype = i
+    L.kratos_hydro_get_kernel.argtypes = [vp, ip]
     L.kratos_hydro_set_zchunk.restype = i
     L.kratos_hydro_set_zchunk.argtypes = [vp, i]
     L.kratos_hydro_set_state.restype = i
@@ -175,6 +177,11 @@ class KratosHydro:
 
     def set_kernel(self, variant):
         _check(self._L.kratos_hydro_set_kernel(self._h, int(variant)))
+
+    def get_kernel(self):
+        v = ctypes.c_int(0)
+        _check(self._L.kratos_hydro_get_kernel(self._h, ctypes.byref(v)))
+        return v.value
 
     def set_zchunk(self, planes):
         _check(self._L.kratos_hydro_set_zchunk(self._h, int(planes)))

@@ -475,6 +475,13 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
     return KRATOS_OK;
 }
 
+int kratos_hydro_get_kernel(kratos_hydro_t* h, int* variant)
+{
+    if (!h || !variant) return fail(KRATOS_ERR_ARG, "NULL argument");
+    *variant = h->variant;
+    return KRATOS_OK;
+}
+
 int kratos_hydro_set_zchunk(kratos_hydro_t* h, int planes)
 {
     if (!h || planes < 0) return fail(KRATOS_ERR_ARG, "bad argument");
