@@ -88,20 +88,24 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(workload_name: str, precision: str, kernel: str):
-    """DRAM bytes per launch (read + write) of `kernel` from the committed ncu --set full capture
-    (profiles/traffic.csv, written from the capture named in its `source` column), or None."""
+def ncu_traffic(workload_name: str, precision: str, integrator: str, kernel: str):
+    """(DRAM bytes per launch (read + write), where it was measured) of `kernel` from the committed
+    ncu --set full captures (profiles/traffic.csv: one row per captured launch, keyed by workload, precision,
+    integrator and the kernel name this file prints; `source` names the summary and `commit` the code it was
+    captured on), or (None, None) when that combination was never captured.  The number is a property of the
+    kernel at that commit, not of this run: the line says so in `traffic_source`."""
     import csv
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path) as f:
             for row in csv.DictReader(f):
                 if (row["workload"] == workload_name and row["precision"] == precision
-                        and kernel.replace(" ", "") in row["kernel"].replace(" ", "")):
-                    return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+                        and row["integrator"] == integrator and row["bench_kernel"] == kernel):
+                    return (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]),
+                            f"profiles/{row['source']} (ncu --set full, commit {row['commit']})")
     except Exception:
         pass
-    return None
+    return None, None
 
 
 class ClockSampler:
@@ -295,9 +299,9 @@ def run_ours(args):
     roofline = None
     if dom:
         kname = kernel_name(resolved, prec, int(dom[-1]), 3 if nz > 1 else (2 if ny > 1 else 1), vanleer)
+        traffic, traffic_src = ncu_traffic(args.workload, args.precision, args.integrator, kname)
         roofline = {"bound": "hbm", "kernel": kname, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
-                    "unit": "GB/s", "frac": kern[dom]["frac"],
-                    "traffic": ncu_traffic(args.workload, args.precision, kname),
+                    "unit": "GB/s", "frac": kern[dom]["frac"], "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "bytes_per_cell": bpc[dom]}
     step_frac = value / world * step_bytes / (peak * 1e9)
 
