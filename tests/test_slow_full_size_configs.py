@@ -12,7 +12,9 @@ kernel and slab height `auto` picks = what bench.py times) against the fp64 CPU 
 Minutes of oracle time on the host cores (C2 and C4 about two minutes each): marked `slow`.  The file name sorts
 last so that the quick parity matrix runs first.
 """
+import json
 import math
+import os
 
 import numpy as np
 import pytest
@@ -41,6 +43,19 @@ def gpu_run(pr, prec, until=None, kernel=binding.KERNEL_AUTO):
     return Ug, t, n, hits, T0, T1
 
 
+def record(config, prec, errors, extra=None):
+    """Measured errors of a full-size comparison, appended to gpurun_out/parity_full_size.jsonl (the folder that
+    comes back from the GPU box; profiles/r2_parity_full_size.md is written from it).  No-op elsewhere."""
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if not os.path.isdir(out):
+        return
+    l1, mx = errors
+    row = {"config": config, "precision": {MIXED: "mixed", FP64: "fp64"}[prec], "rel_l1_max": max(l1), "pointwise_max": max(mx)}
+    row.update(extra or {})
+    with open(os.path.join(out, "parity_full_size.jsonl"), "a") as f:
+        f.write(json.dumps(row) + "\n")
+
+
 def drift(T0, T1, U):
     A0 = np.array([math.fsum(np.abs(U[m]).ravel()) for m in range(5)])
     return float((np.abs(T1 - T0) / np.maximum(np.maximum(np.abs(T0), A0), 1e-300)).max())   # (unused momenta: 0 / tiny)
@@ -57,7 +72,7 @@ def test_c1_all_seeds(seed, prec):
     assert hits == 0 and hits_o == 0
     assert tg == pytest.approx(0.2, abs=1e-15)
     assert abs(ng - no) <= (0 if prec == FP64 else 1)
-    assert_parity(Ug, Uo, prec, what=f"C1 seed {seed}")
+    record("C1 256 cells to t=0.2", prec, assert_parity(Ug, Uo, prec, what=f"C1 seed {seed}"), {"seed": seed, "steps": ng})
 
 
 # --------------------------------------------------------------------------- C2
@@ -81,8 +96,10 @@ def test_c2_full_period(c2_oracle, prec):
     Ug, tg, ng, hits, T0, T1 = gpu_run(pr, prec, until=1.0)
     assert tg == 1.0 and hits == 0
     assert abs(ng - no) <= (0 if prec == FP64 else 2)
-    assert_parity(Ug, Uo, prec, what="C2 512^2, one period")
+    err = assert_parity(Ug, Uo, prec, what="C2 512^2, one period")
     assert drift(T0, T1, pr.U) <= 1e-13
+    record("C2 512^2 one period", prec, err, {"steps": ng, "drift": drift(T0, T1, pr.U), "eq6_density_gpu": eq6_l1(Ug[0], pr.U[0]),
+                                              "eq6_density_oracle": eq6_l1(Uo[0], pr.U[0])})
     # back at the initial state after one crossing time: the Eq. 6 error of the density is the
     # scheme's own truncation error, the same number on both sides, and falls as ~N^-2 (the oracle
     # alone gives 1.98e-2, 5.55e-3, 1.53e-3 at N = 64, 128, 256 for this diagonal wave: a factor 3.6 per doubling)
@@ -106,8 +123,9 @@ def test_c3_full_size(c3_oracle, prec):
     pr, Uo = c3_oracle
     Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
     assert hits == 0
-    assert_parity(Ug, Uo, prec, what="C3 2048^2, 100 steps")
+    err = assert_parity(Ug, Uo, prec, what="C3 2048^2, 100 steps")
     assert drift(T0, T1, pr.U) <= 1e-13
+    record("C3 2048^2 100 steps", prec, err, {"steps": 100, "drift": drift(T0, T1, pr.U)})
 
 
 # --------------------------------------------------------------------------- C4
@@ -125,7 +143,8 @@ def test_c4_full_size(c4_oracle, prec):
     pr, Uo = c4_oracle
     Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
     assert hits == 0
-    assert_parity(Ug, Uo, prec, what="C4 256^3, 50 steps")
+    record("C4 256^3 50 steps", prec, assert_parity(Ug, Uo, prec, what="C4 256^3, 50 steps"),
+           {"steps": 50, "drift": float(max(abs(T1[0] - T0[0]) / T0[0], abs(T1[4] - T0[4]) / T0[4])), "floor_hits": hits})
     # the ambient gas at the edges is still at rest: mass and energy leave through no face
     assert abs(T1[0] - T0[0]) <= 1e-13 * T0[0] and abs(T1[4] - T0[4]) <= 1e-13 * T0[4]
 
@@ -144,8 +163,9 @@ def test_c5_recipe_at_256_cell_by_cell(c5_256_oracle, prec):
     pr, Uo = c5_256_oracle
     Ug, _, _, hits, T0, T1 = gpu_run(pr, prec)
     assert hits == 0
-    assert_parity(Ug, Uo, prec, what="C5 recipe at 256^3, 20 steps")
+    err = assert_parity(Ug, Uo, prec, what="C5 recipe at 256^3, 20 steps")
     assert drift(T0, T1, pr.U) <= 1e-13
+    record("C5 recipe at 256^3 20 steps, cell by cell", prec, err, {"steps": 20, "drift": drift(T0, T1, pr.U)})
 
 
 def test_c5_full_size_all_20_steps_sampled():
@@ -192,4 +212,5 @@ def test_c5_full_size_all_20_steps_sampled():
         ref = sub[:, halo:halo + core, halo:halo + core, halo:halo + core]
         kc, jc, ic = np.arange(k0, k0 + core) % n, np.arange(j0, j0 + core) % n, np.arange(i0, i0 + core) % n
         got = Ug[:, kc][:, :, jc][:, :, :, ic]
-        assert_parity(got, ref, MIXED, what=f"C5 512^3 core at {(k0, j0, i0)}")
+        record("C5 512^3 20 steps, sampled 12^3 core", MIXED, assert_parity(got, ref, MIXED, what=f"C5 512^3 core at {(k0, j0, i0)}"),
+               {"steps": nstep, "core_at": [k0, j0, i0], "drift": drift(T0, T1, pr.U)})
