@@ -4,7 +4,8 @@
  * The library advances the compressible Euler equations (Eq. 2)
  *     d_t rho + div(rho v) = 0,  d_t(rho v) + div(rho v v + p I) = 0,  d_t eps + div[(eps+p) v] = 0,
  *     eps = p/(gamma-1) + rho v^2/2
- * on ONE uniform Cartesian block on ONE GPU with the paper's default scheme: primitive
+ * on ONE uniform Cartesian block on ONE GPU (several such blocks can be stacked along z, one per GPU, through
+ * communication boundaries: see the end of this file) with the paper's default scheme: primitive
  * recovery (Sec. 3.1), ghost zones by the paper's boundary rules
  * (Sec. 3.1.1), minmod-limited PLM (Eq. 3), the
  * subtraction-safe HLLC solver (Eq. 4-5), a flux-difference update inside
@@ -78,6 +79,10 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
 #define KRATOS_BC_FREE 1     /* q(-i-1/2) = q(1/2) */
 #define KRATOS_BC_OUTFLOW 2  /* Free, but inward normal velocity v(-i-1/2) = min(v(1/2), 0) */
 #define KRATOS_BC_REFLECT 3  /* q(-i-1/2) = q(i+1/2), normal velocity negated */
+#define KRATOS_BC_COMM 4     /* communication boundary onto ANOTHER block (Sec. 3.1.2: "c-boundaries"): the two
+                                ghost planes beyond the face are supplied by the block on the other side.  z faces only;
+                                mixed precision, Heun, blocks the TMA kernel serves (nx % 32 == 0, ny % 16 == 0), nz >= 4.
+                                See "Communication boundaries" below. */
 
 /* kernel variants (kratos_hydro_set_kernel) */
 #define KRATOS_KERNEL_AUTO 0   /* x,y active: TMA (mixed, 3D, nx % 32 == 0, ny % 16 == 0), strip (mixed, 2D, even extents),
@@ -174,6 +179,67 @@ KRATOS_API int kratos_hydro_launch_count(kratos_hydro_t *h, long long *n);
  * ms, launches: host arrays of 3.  Synchronises. */
 KRATOS_API int kratos_hydro_set_profiling(kratos_hydro_t *h, int enable);
 KRATOS_API int kratos_hydro_get_timing(kratos_hydro_t *h, double ms[3], long long launches[3]);
+
+/* ---- Communication boundaries: one block per GPU, blocks stacked along z (Sec. 3.1.2; Table 2's
+ * two-GPU splits).
+ *
+ * A z face with KRATOS_BC_COMM has a ghost array per state array, [5][2][ny][nx] doubles (field, plane, y, x; plane 0 is
+ * the one further from the block on the low side and the one next to it on the high side: ghost planes in ascending z),
+ * which the block on the other side fills: its stage kernels store every updated plane that lies within two planes of the
+ * common face a second time, straight into this array (peer memory: the same process, or another process through a CUDA IPC
+ * handle; over NVLink between GPUs) -- the halo exchange is fused into the stage kernel, there is no pack / send / unpack.
+ * What remains for the driver (paper_2501_02317_b200/slab.py) is ordering: a block may start stage 2 only after its
+ * neighbours have finished stage 1, and the next step's stage 1 only after their stage 2; and the time step is the minimum
+ * over all blocks.  Hence the step is cut into pieces:
+ *
+ *     set_state on every block; get_/set_reference_pressure (one value for all blocks); push_halo; <sync>
+ *     begin_run(cfl, t0)                       local CFL rate
+ *     repeat:  get_rate -> <max over blocks> -> set_rate;  substep(PREPARE);  substep(STAGE1);  <sync>;  substep(STAGE2);  <sync>
+ *     end_run
+ *
+ * <sync> = every block's stream has passed this point before any continues (stream order within a process, a collective
+ * of the process group across processes).  kratos_hydro_step / run / run_until refuse blocks with communication boundaries.
+ * array: 0 = the current state, 1 = the predictor of the Heun step.  side: 0 = low z face, 1 = high z face. */
+#define KRATOS_PHASE_PREPARE 0 /* dt = cfl / rate (the rate set by set_rate, or left by the last stage 2), t += dt */
+#define KRATOS_PHASE_STAGE1 1
+#define KRATOS_PHASE_STAGE2 2
+
+/* Device pointer of this block's ghost array (owned by the handle).  ptr: host. */
+KRATOS_API int kratos_hydro_ghost_array(kratos_hydro_t *h, int array, int side, double **ptr);
+
+/* CUDA IPC handle (64 bytes, cudaIpcMemHandle_t) of that ghost array, for a neighbour in another process.  handle: host. */
+KRATOS_API int kratos_hydro_ghost_ipc_handle(kratos_hydro_t *h, int array, int side, unsigned char handle[64]);
+
+/* The block beyond z face `side`: its ghost arrays that hold THIS block's planes (its high-side arrays for side 0, its
+ * low-side arrays for side 1) of the current state and of the predictor, as device pointers valid on this handle's device
+ * (the caller keeps them alive).  open_peer takes the neighbour's IPC handles instead and maps them (unmapped at destroy). */
+KRATOS_API int kratos_hydro_set_peer(kratos_hydro_t *h, int side, double *peer_ghost_state, double *peer_ghost_pred);
+KRATOS_API int kratos_hydro_open_peer(kratos_hydro_t *h, int side, const unsigned char handle_state[64],
+                                      const unsigned char handle_pred[64]);
+
+/* Copy the two planes of the current state next to each communication boundary into the neighbours' ghost arrays (after
+ * set_state; during a run the stage kernels do this themselves).  Asynchronous. */
+KRATOS_API int kratos_hydro_push_halo(kratos_hydro_t *h);
+
+/* The pieces of kratos_hydro_run (see above).  begin_run: Courant number and start time, CFL rate of the current state if
+ * none is at hand.  substep: one KRATOS_PHASE_*; asynchronous.  end_run: time reached and steps taken (host; steps_done may
+ * be NULL); synchronises; KRATOS_ERR_NONFINITE as for run.  Heun integrator, mixed or all-fp64 precision; also valid for
+ * blocks without communication boundaries (then equal to run). */
+KRATOS_API int kratos_hydro_begin_run(kratos_hydro_t *h, double cfl, double t0);
+KRATOS_API int kratos_hydro_substep(kratos_hydro_t *h, int phase);
+KRATOS_API int kratos_hydro_end_run(kratos_hydro_t *h, double *t, int *steps_done);
+
+/* The CFL rate maximum max_cells sum_d (|v_d| + c)/dx_d of the current state as left by begin_run, cfl_dt or
+ * the last stage 2, and its replacement by the maximum over all blocks.  rate: one double, host (synchronises) or device
+ * (asynchronous, on the handle's stream). */
+KRATOS_API int kratos_hydro_get_rate(kratos_hydro_t *h, double *rate, int on_device);
+KRATOS_API int kratos_hydro_set_rate(kratos_hydro_t *h, const double *rate, int on_device);
+
+/* Reference pressure of the mixed-precision solver (see the top of this file; 0 in the other modes).  get computes it from
+ * the current state if that has not happened yet.  set replaces it (rounded to fp32; >= 0) until the next set_state: blocks
+ * of one decomposed domain must share one value (reading S17).  p_ref: host.  Both synchronise. */
+KRATOS_API int kratos_hydro_get_reference_pressure(kratos_hydro_t *h, double *p_ref);
+KRATOS_API int kratos_hydro_set_reference_pressure(kratos_hydro_t *h, double p_ref);
 
 /* Message of the last error raised on this thread ("" if none).  Never NULL. */
 KRATOS_API const char *kratos_hydro_last_error(void);

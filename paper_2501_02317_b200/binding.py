@@ -17,7 +17,8 @@ import numpy as np
 from . import build as _build
 
 PREC_MIXED, PREC_FP64, PREC_SINGLE = 0, 1, 2
-BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT = 0, 1, 2, 3
+BC_PERIODIC, BC_FREE, BC_OUTFLOW, BC_REFLECT, BC_COMM = 0, 1, 2, 3, 4
+PHASE_PREPARE, PHASE_STAGE1, PHASE_STAGE2 = 0, 1, 2
 INTEGRATOR_HEUN, INTEGRATOR_VANLEER = 0 << 4, 1 << 4   # scheme word bits 4-5
 KERNEL_AUTO, KERNEL_SIMPLE, KERNEL_TILED, KERNEL_PAIRED, KERNEL_TMA, KERNEL_STRIP = 0, 1, 2, 3, 5, 6
 OK, ERR_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONFINITE = 0, -1, -2, -3, -4
@@ -29,6 +30,11 @@ SYMBOLS = [
     "kratos_hydro_cfl_dt", "kratos_hydro_step", "kratos_hydro_run", "kratos_hydro_run_until",
     "kratos_hydro_totals", "kratos_hydro_floor_hits", "kratos_hydro_status", "kratos_hydro_launch_count",
     "kratos_hydro_set_profiling", "kratos_hydro_get_timing", "kratos_hydro_last_error", "kratos_hydro_version",
+    # communication boundaries and the pieces of a run (multi-block driver: slab.py)
+    "kratos_hydro_ghost_array", "kratos_hydro_ghost_ipc_handle", "kratos_hydro_set_peer", "kratos_hydro_open_peer",
+    "kratos_hydro_push_halo", "kratos_hydro_begin_run", "kratos_hydro_substep", "kratos_hydro_end_run",
+    "kratos_hydro_get_rate", "kratos_hydro_set_rate", "kratos_hydro_get_reference_pressure",
+    "kratos_hydro_set_reference_pressure",
 ]
 
 _lib = None
@@ -93,6 +99,31 @@ def load() -> ctypes.CDLL:
     L.kratos_hydro_set_profiling.argtypes = [vp, i]
     L.kratos_hydro_get_timing.restype = i
     L.kratos_hydro_get_timing.argtypes = [vp, dp, llp]
+    ucp = ctypes.POINTER(ctypes.c_ubyte)
+    L.kratos_hydro_ghost_array.restype = i
+    L.kratos_hydro_ghost_array.argtypes = [vp, i, i, ctypes.POINTER(vp)]
+    L.kratos_hydro_ghost_ipc_handle.restype = i
+    L.kratos_hydro_ghost_ipc_handle.argtypes = [vp, i, i, ucp]
+    L.kratos_hydro_set_peer.restype = i
+    L.kratos_hydro_set_peer.argtypes = [vp, i, vp, vp]
+    L.kratos_hydro_open_peer.restype = i
+    L.kratos_hydro_open_peer.argtypes = [vp, i, ucp, ucp]
+    L.kratos_hydro_push_halo.restype = i
+    L.kratos_hydro_push_halo.argtypes = [vp]
+    L.kratos_hydro_begin_run.restype = i
+    L.kratos_hydro_begin_run.argtypes = [vp, d, d]
+    L.kratos_hydro_substep.restype = i
+    L.kratos_hydro_substep.argtypes = [vp, i]
+    L.kratos_hydro_end_run.restype = i
+    L.kratos_hydro_end_run.argtypes = [vp, dp, ip]
+    L.kratos_hydro_get_rate.restype = i
+    L.kratos_hydro_get_rate.argtypes = [vp, vp, i]
+    L.kratos_hydro_set_rate.restype = i
+    L.kratos_hydro_set_rate.argtypes = [vp, vp, i]
+    L.kratos_hydro_get_reference_pressure.restype = i
+    L.kratos_hydro_get_reference_pressure.argtypes = [vp, dp]
+    L.kratos_hydro_set_reference_pressure.restype = i
+    L.kratos_hydro_set_reference_pressure.argtypes = [vp, d]
     L.kratos_hydro_last_error.restype = ctypes.c_char_p
     L.kratos_hydro_last_error.argtypes = []
     L.kratos_hydro_version.restype = ctypes.c_char_p
@@ -252,3 +283,66 @@ class KratosHydro:
         n = (ctypes.c_longlong * 3)()
         _check(self._L.kratos_hydro_get_timing(self._h, ms, n))
         return {k: (ms[i], n[i]) for i, k in enumerate(("stage1", "stage2", "other"))}
+
+    # -- communication boundaries and the pieces of a run (include/kratos_hydro.h, "Communication boundaries")
+    def ghost_array(self, array, side):
+        """Device address of this block's ghost array (int)."""
+        p = ctypes.c_void_p(0)
+        _check(self._L.kratos_hydro_ghost_array(self._h, int(array), int(side), ctypes.byref(p)))
+        return int(p.value)
+
+    def ghost_ipc_handle(self, array, side):
+        """The 64 bytes of the CUDA IPC handle of that ghost array."""
+        buf = (ctypes.c_ubyte * 64)()
+        _check(self._L.kratos_hydro_ghost_ipc_handle(self._h, int(array), int(side), buf))
+        return bytes(buf)
+
+    def set_peer(self, side, peer_ghost_state, peer_ghost_pred):
+        _check(self._L.kratos_hydro_set_peer(self._h, int(side), ctypes.c_void_p(int(peer_ghost_state)),
+                                             ctypes.c_void_p(int(peer_ghost_pred))))
+
+    def open_peer(self, side, handle_state, handle_pred):
+        a = (ctypes.c_ubyte * 64).from_buffer_copy(bytes(handle_state))
+        b = (ctypes.c_ubyte * 64).from_buffer_copy(bytes(handle_pred))
+        _check(self._L.kratos_hydro_open_peer(self._h, int(side), a, b))
+
+    def push_halo(self):
+        _check(self._L.kratos_hydro_push_halo(self._h))
+
+    def begin_run(self, cfl, t0=0.0):
+        _check(self._L.kratos_hydro_begin_run(self._h, float(cfl), float(t0)))
+
+    def substep(self, phase):
+        _check(self._L.kratos_hydro_substep(self._h, int(phase)))
+
+    def end_run(self):
+        t = ctypes.c_double(0.0)
+        n = ctypes.c_int(0)
+        _check(self._L.kratos_hydro_end_run(self._h, ctypes.byref(t), ctypes.byref(n)))
+        return t.value, n.value
+
+    def get_rate(self, out=None):
+        """The CFL rate maximum: a float, or written into a 1-element float64 tensor / array (device: asynchronous)."""
+        if out is None:
+            v = ctypes.c_double(0.0)
+            _check(self._L.kratos_hydro_get_rate(self._h, ctypes.cast(ctypes.byref(v), ctypes.c_void_p), 0))
+            return v.value
+        ptr, dev, _keep = _buffer(out)
+        _check(self._L.kratos_hydro_get_rate(self._h, ctypes.c_void_p(ptr), dev))
+        return out
+
+    def set_rate(self, rate):
+        if isinstance(rate, (int, float)):
+            v = ctypes.c_double(float(rate))
+            _check(self._L.kratos_hydro_set_rate(self._h, ctypes.cast(ctypes.byref(v), ctypes.c_void_p), 0))
+            return
+        ptr, dev, _keep = _buffer(rate)
+        _check(self._L.kratos_hydro_set_rate(self._h, ctypes.c_void_p(ptr), dev))
+
+    def get_reference_pressure(self):
+        v = ctypes.c_double(0.0)
+        _check(self._L.kratos_hydro_get_reference_pressure(self._h, ctypes.byref(v)))
+        return v.value
+
+    def set_reference_pressure(self, p_ref):
+        _check(self._L.kratos_hydro_set_reference_pressure(self._h, float(p_ref)))

@@ -64,6 +64,13 @@ struct kratos_hydro {
     double* stage_buf;  // Single mode: staging area for the double <-> float conversion of host states (device, on demand)
     int tot_blocks;
     cudaStream_t stream;
+    // communication boundaries in z (KRATOS_BC_COMM): ghost arrays [5][2][ny][nx] of the two state arrays beyond the
+    // low / high face ([array][side]), the neighbours' ghost arrays this block's stage kernels store into, and what was
+    // opened from CUDA IPC handles (closed at destroy)
+    bool comm[2];
+    double* ghost[2][2];
+    double* peer[2][2];
+    void* ipc_opened[2][2];
     int device;       // CUDA device the handle lives on (every entry point runs with it current)
     bool rate_valid;  // ctrl->rate_bits holds the rate maximum of U0
     bool pref_valid;  // ctrl->p_ref was computed from the state last given to set_state
@@ -138,6 +145,7 @@ void collect_timing(kratos_hydro* h)
 
 int auto_variant(const kratos_hydro* h)
 {
+    if (h->comm[0] || h->comm[1]) return KRATOS_KERNEL_TMA;   // checked at create: the only kernel that serves them
     if (h->integ == 1) return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;  // van Leer
     if (h->prec == KRATOS_PREC_SINGLE)   // all-fp32 state: the TMA kernel on float boxes, else the general kernel
         return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;
@@ -328,7 +336,8 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         if (n[d] > 1) {
             nactive++;
             const int lo = bc[2 * d], hi = bc[2 * d + 1];
-            if (lo < 0 || lo > 3 || hi < 0 || hi > 3) { fail(KRATOS_ERR_ARG, "bad bc code on axis %d", d); return nullptr; }
+            const int top = (d == 2) ? KRATOS_BC_COMM : KRATOS_BC_REFLECT;   // communication boundaries: z faces only
+            if (lo < 0 || lo > top || hi < 0 || hi > top) { fail(KRATOS_ERR_ARG, "bad bc code on axis %d", d); return nullptr; }
             if ((lo == KRATOS_BC_PERIODIC) != (hi == KRATOS_BC_PERIODIC)) {
                 fail(KRATOS_ERR_ARG, "periodic on one side only of axis %d", d);
                 return nullptr;
@@ -364,6 +373,16 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->tiled_ok = g.active[0] && g.active[1] && integ == 0;   // the fused stage kernels are the Heun path
     h->maps = nullptr;
     h->smaps = nullptr;
+    for (int side = 0; side < 2; side++) {
+        h->comm[side] = g.active[2] && g.bc[4 + side] == KRATOS_BC_COMM;
+        for (int a = 0; a < 2; a++) { h->ghost[a][side] = nullptr; h->peer[a][side] = nullptr; h->ipc_opened[a][side] = nullptr; }
+    }
+    if ((h->comm[0] || h->comm[1]) && (prec != KRATOS_PREC_MIXED || integ != 0 || !tma::supported(g) || nz < 4)) {
+        fail(KRATOS_ERR_ARG, "communication boundaries need mixed precision, the Heun integrator, three active axes, "
+                             "nx %% 32 == 0, ny %% 16 == 0 and nz >= 4 (they are served by the TMA kernel)");
+        delete h;
+        return nullptr;
+    }
     h->variant = auto_variant(h);
     h->zchunk = 0;
     h->stream = 0;
@@ -397,6 +416,18 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         kratos_hydro_destroy(h);
         return nullptr;
     }
+    for (int side = 0; side < 2; side++) {
+        if (!h->comm[side]) continue;
+        const size_t gb = sizeof(double) * 5 * 2 * (size_t)nx * ny;
+        for (int a = 0; a < 2; a++) {
+            if ((e = cudaMalloc(&h->ghost[a][side], gb)) != cudaSuccess || (e = cudaMemset(h->ghost[a][side], 0, gb)) != cudaSuccess) {
+                fail(e == cudaErrorMemoryAllocation ? KRATOS_ERR_ALLOC : KRATOS_ERR_CUDA, "create (ghost planes): %s", cudaGetErrorString(e));
+                cudaGetLastError();
+                kratos_hydro_destroy(h);
+                return nullptr;
+            }
+        }
+    }
     tiled_configure();
     pr::configure();
     tma::configure();
@@ -414,6 +445,14 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         h->smaps = new (std::nothrow) strip::StageMaps;
         if (h->smaps) strip::build_maps(h->smaps, h->U0, h->U1, g);
     }
+    if (h->comm[0] || h->comm[1]) {
+        double* none[2] = {nullptr, nullptr};
+        if (!h->maps || !h->maps->ok || !tma::set_comm_maps(h->maps, g, h->ghost[0], h->ghost[1], none, none)) {
+            fail(KRATOS_ERR_CUDA, "create: tensor maps of the ghost planes");
+            kratos_hydro_destroy(h);
+            return nullptr;
+        }
+    }
     h->variant = auto_variant(h);
     return h;
 }
@@ -429,6 +468,11 @@ void kratos_hydro_destroy(kratos_hydro_t* h)
     cudaFree(h->d_tot);
     cudaFree(h->p_partial);
     cudaFree(h->stage_buf);
+    for (int a = 0; a < 2; a++)
+        for (int side = 0; side < 2; side++) {
+            cudaFree(h->ghost[a][side]);
+            if (h->ipc_opened[a][side]) cudaIpcCloseMemHandle(h->ipc_opened[a][side]);
+        }
     if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
     delete h->maps;
     delete h->smaps;
@@ -458,6 +502,8 @@ int kratos_hydro_set_kernel(kratos_hydro_t* h, int variant)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
     if (variant == KRATOS_KERNEL_AUTO) variant = auto_variant(h);
+    if ((h->comm[0] || h->comm[1]) && variant != KRATOS_KERNEL_TMA)
+        return fail(KRATOS_ERR_ARG, "blocks with communication boundaries are served by the TMA kernel only");
     if (h->prec == KRATOS_PREC_SINGLE && variant != auto_variant(h) && variant != KRATOS_KERNEL_SIMPLE)
         return fail(KRATOS_ERR_ARG, "this kernel variant does not serve the all-fp32 mode on this block");
     if ((variant == KRATOS_KERNEL_TILED || variant == KRATOS_KERNEL_PAIRED) && !h->tiled_ok)
@@ -537,6 +583,9 @@ int kratos_hydro_step(kratos_hydro_t* h, double dt)
 {
     if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(KRATOS_ERR_ARG, "dt must be > 0 and finite");
+    if (h->comm[0] || h->comm[1])
+        return fail(KRATOS_ERR_ARG, "a block with communication boundaries advances by kratos_hydro_substep (its neighbours must "
+                                    "have delivered their planes between the stages)");
     DeviceGuard dg(h);
     int rc;
     // first step after set_state: the reference pressure of the mixed-precision kernels comes from this state
@@ -555,6 +604,8 @@ static int run_impl(kratos_hydro_t* h, double cfl, double t_end, int max_steps, 
     if (!h || !t_inout) return fail(KRATOS_ERR_ARG, "NULL argument");
     if (!(cfl > 0.0) || !std::isfinite(cfl) || max_steps < 0) return fail(KRATOS_ERR_ARG, "bad cfl / step count");
     if (!std::isfinite(*t_inout) || !std::isfinite(t_end)) return fail(KRATOS_ERR_ARG, "non-finite time");
+    if (h->comm[0] || h->comm[1])
+        return fail(KRATOS_ERR_ARG, "a block with communication boundaries advances by kratos_hydro_substep");
     DeviceGuard dg(h);
     int rc;
     {
@@ -683,5 +734,186 @@ int kratos_hydro_get_timing(kratos_hydro_t* h, double ms[3], long long launches[
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     collect_timing(h);
     for (int s = 0; s < 3; s++) { ms[s] = h->prof_ms[s]; launches[s] = h->prof_n[s]; }
+    return KRATOS_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Communication boundaries (Sec. 3.1.2) and the pieces of a step a multi-block driver interleaves
+// with its own synchronisation (paper_2501_02317_b200/slab.py).
+
+static int check_ghost_args(kratos_hydro_t* h, int array, int side)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    if (array < 0 || array > 1 || side < 0 || side > 1) return fail(KRATOS_ERR_ARG, "array and side must be 0 or 1");
+    if (!h->comm[side]) return fail(KRATOS_ERR_ARG, "z face %d of this block is no communication boundary", side);
+    return KRATOS_OK;
+}
+
+int kratos_hydro_ghost_array(kratos_hydro_t* h, int array, int side, double** ptr)
+{
+    int rc = check_ghost_args(h, array, side);
+    if (rc) return rc;
+    if (!ptr) return fail(KRATOS_ERR_ARG, "NULL argument");
+    *ptr = h->ghost[array][side];
+    return KRATOS_OK;
+}
+
+int kratos_hydro_ghost_ipc_handle(kratos_hydro_t* h, int array, int side, unsigned char handle[64])
+{
+    int rc = check_ghost_args(h, array, side);
+    if (rc) return rc;
+    if (!handle) return fail(KRATOS_ERR_ARG, "NULL argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    DeviceGuard dg(h);
+    cudaIpcMemHandle_t m;
+    CUDA_TRY(cudaIpcGetMemHandle(&m, h->ghost[array][side]));
+    memcpy(handle, &m, 64);
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_peer(kratos_hydro_t* h, int side, double* peer_ghost_state, double* peer_ghost_pred)
+{
+    int rc = check_ghost_args(h, 0, side);
+    if (rc) return rc;
+    if (!peer_ghost_state || !peer_ghost_pred) return fail(KRATOS_ERR_ARG, "NULL peer array");
+    DeviceGuard dg(h);
+    h->peer[0][side] = peer_ghost_state;
+    h->peer[1][side] = peer_ghost_pred;
+    double* none[2] = {nullptr, nullptr};
+    if (!tma::set_comm_maps(h->maps, h->g, none, none, h->peer[0], h->peer[1]))
+        return fail(KRATOS_ERR_CUDA, "tensor maps of the peer ghost arrays");
+    return KRATOS_OK;
+}
+
+int kratos_hydro_open_peer(kratos_hydro_t* h, int side, const unsigned char handle_state[64], const unsigned char handle_pred[64])
+{
+    int rc = check_ghost_args(h, 0, side);
+    if (rc) return rc;
+    if (!handle_state || !handle_pred) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
+    void* p[2] = {nullptr, nullptr};
+    const unsigned char* hd[2] = {handle_state, handle_pred};
+    for (int a = 0; a < 2; a++) {
+        cudaIpcMemHandle_t m;
+        memcpy(&m, hd[a], 64);
+        if (h->ipc_opened[a][side]) { cudaIpcCloseMemHandle(h->ipc_opened[a][side]); h->ipc_opened[a][side] = nullptr; }
+        CUDA_TRY(cudaIpcOpenMemHandle(&p[a], m, cudaIpcMemLazyEnablePeerAccess));
+        h->ipc_opened[a][side] = p[a];
+    }
+    return kratos_hydro_set_peer(h, side, (double*)p[0], (double*)p[1]);
+}
+
+static int peers_ready(kratos_hydro_t* h)
+{
+    for (int side = 0; side < 2; side++)
+        if (h->comm[side] && (!h->peer[0][side] || !h->peer[1][side]))
+            return fail(KRATOS_ERR_ARG, "z face %d is a communication boundary without a peer (kratos_hydro_set_peer / _open_peer)", side);
+    return KRATOS_OK;
+}
+
+int kratos_hydro_push_halo(kratos_hydro_t* h)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    int rc = peers_ready(h);
+    if (rc) return rc;
+    DeviceGuard dg(h);
+    const Grid& g = h->g;
+    const size_t plane = (size_t)g.n[0] * g.n[1];
+    for (int side = 0; side < 2; side++) {
+        if (!h->comm[side]) continue;
+        const size_t first = side == 0 ? 0 : (size_t)(g.n[2] - 2) * plane;   // the two planes next to the face
+        for (int f = 0; f < 5; f++)
+            CUDA_TRY(cudaMemcpyAsync(h->peer[0][side] + (size_t)f * 2 * plane, h->U0 + (size_t)f * g.N + first,
+                                     sizeof(double) * 2 * plane, cudaMemcpyDefault, h->stream));
+    }
+    return KRATOS_OK;
+}
+
+int kratos_hydro_begin_run(kratos_hydro_t* h, double cfl, double t0)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    if (!(cfl > 0.0) || !std::isfinite(cfl) || !std::isfinite(t0)) return fail(KRATOS_ERR_ARG, "bad cfl / time");
+    DeviceGuard dg(h);
+    int rc;
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        configure_run_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, cfl, 0.0, t0);
+    }
+    if ((!h->rate_valid || !h->pref_valid) && (rc = launch_cfl_rate(h))) return rc;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_substep(kratos_hydro_t* h, int phase)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    if (h->integ != 0 || h->prec == KRATOS_PREC_SINGLE) return fail(KRATOS_ERR_ARG, "substep serves the Heun integrator on an fp64 state");
+    DeviceGuard dg(h);
+    int rc;
+    if (phase == KRATOS_PHASE_PREPARE) {
+        if (!h->rate_valid || !h->pref_valid) return fail(KRATOS_ERR_ARG, "substep before kratos_hydro_begin_run");
+        LaunchTimer lt(h, SLOT_OTHER);
+        prepare_step_kernel<<<1, 1, 0, h->stream>>>(h->ctrl);
+        return KRATOS_OK;
+    }
+    if (phase != KRATOS_PHASE_STAGE1 && phase != KRATOS_PHASE_STAGE2) return fail(KRATOS_ERR_ARG, "bad phase");
+    if ((rc = peers_ready(h))) return rc;
+    rc = (h->prec == KRATOS_PREC_MIXED) ? launch_stage<float>(h, phase) : launch_stage<double>(h, phase);
+    if (rc == KRATOS_OK && phase == KRATOS_PHASE_STAGE2) h->rate_valid = true;
+    return rc;
+}
+
+int kratos_hydro_end_run(kratos_hydro_t* h, double* t, int* steps_done)
+{
+    if (!h || !t) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
+    int rc = read_ctrl(h);
+    if (rc) return rc;
+    *t = h->h_ctrl->t;
+    if (steps_done) *steps_done = (int)h->h_ctrl->steps;
+    if (h->h_ctrl->nonfinite) return fail(KRATOS_ERR_NONFINITE, "non-finite time step during run (t = %g)", h->h_ctrl->t);
+    return KRATOS_OK;
+}
+
+int kratos_hydro_get_rate(kratos_hydro_t* h, double* rate, int on_device)
+{
+    if (!h || !rate) return fail(KRATOS_ERR_ARG, "NULL argument");
+    if (!h->rate_valid) return fail(KRATOS_ERR_ARG, "no CFL rate at hand (kratos_hydro_begin_run / cfl_dt / a stage 2 first)");
+    DeviceGuard dg(h);
+    CUDA_TRY(cudaMemcpyAsync(rate, &h->ctrl->rate_bits, sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_rate(kratos_hydro_t* h, const double* rate, int on_device)
+{
+    if (!h || !rate) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
+    CUDA_TRY(cudaMemcpyAsync(&h->ctrl->rate_bits, rate, sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    if (!on_device) CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->rate_valid = true;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_get_reference_pressure(kratos_hydro_t* h, double* p_ref)
+{
+    if (!h || !p_ref) return fail(KRATOS_ERR_ARG, "NULL argument");
+    DeviceGuard dg(h);
+    int rc;
+    if (!h->pref_valid && (rc = launch_cfl_rate(h))) return rc;
+    if ((rc = read_ctrl(h))) return rc;
+    *p_ref = h->prec == KRATOS_PREC_MIXED ? h->h_ctrl->p_ref : 0.0;
+    return KRATOS_OK;
+}
+
+int kratos_hydro_set_reference_pressure(kratos_hydro_t* h, double p_ref)
+{
+    if (!h) return fail(KRATOS_ERR_ARG, "NULL handle");
+    const float m = (float)p_ref;   // the fp64 recovery and the fp32 solver must use the very same number
+    if (!(m >= 0.0f) || !(m < 3.0e38f)) return fail(KRATOS_ERR_ARG, "reference pressure must be >= 0 and finite in fp32");
+    DeviceGuard dg(h);
+    const double v = (double)m;
+    CUDA_TRY(cudaMemcpyAsync(&h->ctrl->p_ref, &v, sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->pref_valid = true;
     return KRATOS_OK;
 }

@@ -13,7 +13,8 @@
 
 namespace kh {
 
-enum : int { BC_PERIODIC = 0, BC_FREE = 1, BC_OUTFLOW = 2, BC_REFLECT = 3 };
+enum : int { BC_PERIODIC = 0, BC_FREE = 1, BC_OUTFLOW = 2, BC_REFLECT = 3,
+             BC_COMM = 4 };   // communication boundary (Sec. 3.1.2): ghost planes supplied by the neighbouring block
 // what a boundary rule does to the normal velocity of a ghost cell
 enum : int { VN_KEEP = 0, VN_NEGATE = 1, VN_MIN0 = 2, VN_MAX0 = 3 };
 

@@ -111,6 +111,11 @@ struct Maps {
     CUtensorMap in_own, in_rows, in_cols;   // stage input: tile box, halo row pair, halo column pair
     CUtensorMap u0_own;                     // U0 (stage 2)
     CUtensorMap out_own;                    // stage output
+    // communication boundaries in z (BC_COMM; Sec. 3.1.2): the two ghost planes of the stage input
+    // beyond the low / high z face (arrays [5][2][ny][nx] the neighbouring block fills), and the neighbours' ghost
+    // arrays of the stage OUTPUT (peer memory), into which this block stores its two planes next to the face
+    CUtensorMap in_glo, in_ghi;
+    CUtensorMap out_plo, out_phi;
 };
 
 // ---- PTX wrappers -------------------------------------------------------------------------------------
@@ -815,7 +820,23 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             int rz;
             const int sk = bc_source(p, nz, g.bc[4], g.bc[5], rz);
             mbar_expect_tx(&sm.full_raw[slot], RAW_TX);
-            tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);   // (slot stride follows the type)
+            // ghost planes of a communication boundary come from the array the neighbouring block has filled
+            // (planes further out than two are loaded for the straight-line code only and never used)
+            if (p < 0 && g.bc[4] == BC_COMM)
+                tma_load4(&sm.raw[slot][0][0][0], &maps.in_glo, i0, j0, max(p + 2, 0), 0, &sm.full_raw[slot]);
+            else if (p >= nz && g.bc[5] == BC_COMM)
+                tma_load4(&sm.raw[slot][0][0][0], &maps.in_ghi, i0, j0, min(p - nz, 1), 0, &sm.full_raw[slot]);
+            else
+                tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);   // (slot stride follows the type)
+        };
+        // The updated plane p leaves by one TMA store; next to a communication boundary the same box is also stored into
+        // the neighbouring block's ghost array over NVLink / peer memory: the halo exchange of Sec. 3.1.2 is part of the
+        // stage kernel (no separate pack / send / unpack pass, no extra read of the state).
+        auto store_plane = [&](int p, const void* src) {
+            tma_store4(&maps.out_own, i0, j0, p, 0, src);
+            if (g.bc[4] == BC_COMM && p < 2) tma_store4(&maps.out_plo, i0, j0, p, 0, src);
+            if (g.bc[5] == BC_COMM && p >= nz - 2) tma_store4(&maps.out_phi, i0, j0, p - (nz - 2), 0, src);
+            tma_commit();
         };
         auto load_halo = [&](int p, int slot) {  // p in [kbeg, kend): an interior plane
             unsigned long long* bar = &sm.full_halo[slot];
@@ -847,10 +868,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 const bool stored = k - 1 >= kbeg;
                 if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
                 if (k - 1 + NSLOT <= plast) load_raw(k - 1 + NSLOT, s_prev);
-                if (stored) {
-                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.u0[(k - 1 - kbeg) % NU0][0][0][0]);
-                    tma_commit();
-                }
+                if (stored) store_plane(k - 1, &sm.u0[(k - 1 - kbeg) % NU0][0][0][0]);
                 if (k + 1 < kend) {
                     const int m = (k + 1 - kbeg) % NU0;
                     // this slot held plane k-2, whose store was committed one group before the one just issued
@@ -861,10 +879,7 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             }
             if (MODE != 2 && lane == 0) {
                 const bool stored = k - 1 >= kbeg;
-                if (stored) {  // plane k-1 was updated in place in phase C of the previous iteration
-                    tma_store4(&maps.out_own, i0, j0, k - 1, 0, &sm.raw[s_prev][0][0][0]);
-                    tma_commit();
-                }
+                if (stored) store_plane(k - 1, &sm.raw[s_prev][0][0][0]);  // updated in place in phase C of the previous iteration
                 if (k >= kbeg && k + NHALO < kend) load_halo(k + NHALO, hs);
                 if (STAGE == 2 && k + 1 < kend) {
                     const int m = (k + 1 - kbeg) % NU0;
@@ -889,9 +904,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         __syncwarp();
         block_bar();
         if (lane == 0) {  // the last plane of the slab
-            if (MODE == 2) tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.u0[(kend - 1 - kbeg) % NU0][0][0][0]);
-            else           tma_store4(&maps.out_own, i0, j0, kend - 1, 0, &sm.raw[s_prev][0][0][0]);
-            tma_commit();
+            if (MODE == 2) store_plane(kend - 1, &sm.u0[(kend - 1 - kbeg) % NU0][0][0][0]);
+            else           store_plane(kend - 1, &sm.raw[s_prev][0][0][0]);
             tma_wait_all0();
         }
         __syncwarp();
@@ -926,12 +940,15 @@ inline EncodeTiledFn encode_tiled_fn()
 }
 
 // Tensor map over one conserved state U[5][nz][ny][nx] (fp64, x fastest) with a box of bx x by x 1 x 5.
-inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx, int by)
+// nplanes: z extent of the array (the block's own, or 2 for the ghost arrays of a communication boundary).
+inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx, int by, int nplanes = 0)
 {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
-    const cuuint64_t dims[4] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2], 5};
-    const cuuint64_t strides[3] = {(cuuint64_t)g.n[0] * 8, (cuuint64_t)g.n[0] * g.n[1] * 8, (cuuint64_t)g.N * 8};
+    if (nplanes <= 0) nplanes = g.n[2];
+    const cuuint64_t dims[4] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)nplanes, 5};
+    const cuuint64_t strides[3] = {(cuuint64_t)g.n[0] * 8, (cuuint64_t)g.n[0] * g.n[1] * 8,
+                                   (cuuint64_t)g.n[0] * g.n[1] * nplanes * 8};
     const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 5};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -953,12 +970,42 @@ inline bool make_map_f32(CUtensorMap* m, const float* W, const Grid& g, int bx =
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+struct StageMaps;
+inline void comm_defaults(StageMaps* sm);
+
 // maps of both stages for the two state buffers of a handle: stage 1 reads A writes B, stage 2 reads B, averages with
 // and writes A.
 struct StageMaps {
     Maps s1, s2;
     bool ok;
 };
+
+// Without communication boundaries the four extra maps are never dereferenced; they alias the block's own arrays.
+inline void comm_defaults(StageMaps* sm)
+{
+    sm->s1.in_glo = sm->s1.in_ghi = sm->s1.in_own; sm->s1.out_plo = sm->s1.out_phi = sm->s1.out_own;
+    sm->s2.in_glo = sm->s2.in_ghi = sm->s2.in_own; sm->s2.out_plo = sm->s2.out_phi = sm->s2.out_own;
+}
+
+// Communication boundaries in z (Heun, fp64 state).  ghostA / ghostB [side]: this block's ghost arrays [5][2][ny][nx] of the
+// state arrays A and B beyond its low (0) / high (1) z face; peerA / peerB [side]: the ghost arrays of the block beyond that
+// face which hold THIS block's planes (its high-side ghosts for side 0, its low-side ghosts for side 1), addressable from
+// this device (same process, or opened from a CUDA IPC handle).  NULL entries: that face is no communication boundary.
+inline bool set_comm_maps(StageMaps* sm, const Grid& g, double* const ghostA[2], double* const ghostB[2],
+                          double* const peerA[2], double* const peerB[2])
+{
+    CUtensorMap* in1[2] = {&sm->s1.in_glo, &sm->s1.in_ghi};
+    CUtensorMap* in2[2] = {&sm->s2.in_glo, &sm->s2.in_ghi};
+    CUtensorMap* out1[2] = {&sm->s1.out_plo, &sm->s1.out_phi};
+    CUtensorMap* out2[2] = {&sm->s2.out_plo, &sm->s2.out_phi};
+    for (int side = 0; side < 2; side++) {
+        if (ghostA[side] && !make_map(in1[side], ghostA[side], g, PTX, PTY, 2)) return false;   // stage 1 reads A
+        if (ghostB[side] && !make_map(in2[side], ghostB[side], g, PTX, PTY, 2)) return false;   // stage 2 reads B
+        if (peerB[side] && !make_map(out1[side], peerB[side], g, PTX, PTY, 2)) return false;    // stage 1 writes B
+        if (peerA[side] && !make_map(out2[side], peerA[side], g, PTX, PTY, 2)) return false;    // stage 2 writes A
+    }
+    return true;
+}
 
 inline bool supported(const Grid& g)
 {
@@ -976,6 +1023,7 @@ inline void build_maps(StageMaps* sm, const double* A, const double* B, const Gr
         return;
     sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = b_own;
     sm->s2.in_own = b_own; sm->s2.in_rows = b_rows; sm->s2.in_cols = b_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
+    comm_defaults(sm);
     sm->ok = true;
 }
 
@@ -991,6 +1039,7 @@ inline void build_maps_vl(StageMaps* sm, const double* A, const float* Wh, const
     sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = w_own;
     // corrector: primitive planes and halo boxes from Wh (columns 4 floats = 16 bytes wide), U^n in and out through A
     sm->s2.in_own = w_own; sm->s2.in_rows = w_rows; sm->s2.in_cols = w_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
+    comm_defaults(sm);
     sm->ok = true;
 }
 
@@ -1006,6 +1055,7 @@ inline void build_maps_single(StageMaps* sm, const float* A, const float* B, con
         return;
     sm->s1.in_own = a_own; sm->s1.in_rows = a_rows; sm->s1.in_cols = a_cols; sm->s1.u0_own = a_own; sm->s1.out_own = b_own;
     sm->s2.in_own = b_own; sm->s2.in_rows = b_rows; sm->s2.in_cols = b_cols; sm->s2.u0_own = a_own; sm->s2.out_own = a_own;
+    comm_defaults(sm);
     sm->ok = true;
 }
 
