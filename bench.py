@@ -2,7 +2,8 @@
 """bench.py -- throughput of the Kratos hydro hot path on B200 (cell-updates/s and % of HBM roofline).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload C5|C4|C3|C5-256] [--precision mixed|fp64]
+                    [--workload C5|C4|C3|C5-256] [--precision mixed|fp64|single] [--integrator heun|vanleer]
+                    [--slabs R | --decomposition slab]
 
 A "step" is one full Heun step (both stages: ghost rules, primitive recovery, PLM, HLLC, fp64 update,
 fused CFL reduction) of one synthetic block.  Default workload: BASELINE.json config 5 (512^3 periodic,
@@ -12,6 +13,12 @@ quoted on.  Prints ONE JSON line (rank 0).
 Multi-GPU: the path does not shard in this build (BASELINE.json: one GPU, no collectives), so
 --gpus N runs N independent replicas ("replicas only"); torch.distributed is
 used for the barrier and the max-over-ranks time only.
+
+--slabs R cuts the block into R z slabs that exchange their ghost planes through communication boundaries
+(paper_2501_02317_b200/slab.py), all in this process on this GPU, advanced in lock step:
+what the decomposition costs on one device (the R stage launches of a step run one after the other).  Under torchrun,
+--decomposition slab gives every rank one slab of the ONE block instead of a replica ("scaling": "strong"; NCCL
+all-reduces for the time step and the ordering, CUDA IPC for the neighbours' ghost arrays).
 
 --impl reference times the oracle (oracle/kratos_oracle.c, as it stands) on the host cores on a
 bounded sample of the same workload.
@@ -336,6 +343,125 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slabs(args):
+    """One block as z slabs (row f-4): --slabs R in this process, or one slab per rank under torchrun."""
+    import numpy as np
+    import torch
+    from paper_2501_02317_b200 import binding, slab
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if args.precision != "mixed" or args.integrator != "heun":
+        raise SystemExit("communication boundaries serve the mixed-precision Heun path")
+    pr, wl_name = workload(args.workload)
+    nx, ny, nz = pr.shape
+    ncell = pr.ncell
+    stream = torch.cuda.Stream()
+    nslab = world if world > 1 else args.slabs
+    s = slab.SlabSolver(nx, ny, nz, pr.gamma, pr.bc, world=nslab, stream=stream)
+    if args.zchunk > 0:
+        for b in s.blocks.values():
+            b.set_zchunk(args.zchunk)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    s.set_state(pr.U)
+    t = s.run(pr.cfl, args.warmup, 0.0)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    barrier()
+    for b in s.blocks.values():
+        b.set_profiling(True)
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
+    e0.record(stream)
+    t = s.run(pr.cfl, args.steps, t)
+    e1.record(stream)
+    barrier()
+    w1 = time.time()
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - l0
+    timing = {"stage1": [0.0, 0], "stage2": [0.0, 0]}
+    for b in s.blocks.values():
+        tm = b.get_timing()
+        for k in timing:
+            timing[k][0] += tm[k][0]
+            timing[k][1] += tm[k][1]
+        b.set_profiling(False)
+    clocks = sampler.stop(w0, w1)
+    from paper_2501_02317_b200 import replicas
+    job_s = replicas.job_time(ms * 1e-3)                 # max over ranks of the device time
+    value = ncell * args.steps / job_s                   # ONE block, whatever the number of slabs: strong scaling
+    hits = s.floor_hits()
+    # end to end: the whole block from and to host memory through the driver, one step per round trip
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    barrier()
+    w2 = time.time()
+    for _ in range(e2e_steps):
+        s.set_state(pr.U)
+        s.run(pr.cfl, 1, 0.0)
+        got = s.get_state()
+    barrier()
+    e2e_s = replicas.job_time(time.time() - w2)
+    del got
+    s.destroy()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = measured_peak()
+    planes = 2 * sum(1 for r in range(nslab) for nb in s.dec.neighbours(r) if nb is not None)
+    halo_bytes = 2 * planes * 5 * nx * ny * 8            # both stages: every cut face side receives two planes of 5 fields
+    kern = {}
+    for k in ("stage1", "stage2"):
+        tot_ms, n = timing[k]
+        if n:
+            per_step = tot_ms / (n / len(s.ranks) if len(s.ranks) else 1)   # the slabs of this process run one after the other
+            gbs = BYTES_PER_CELL[k] * ncell / world / (per_step * 1e-3) / 1e9
+            kern[k] = {"avg_ms": per_step, "launches": n, "algorithmic_bytes": BYTES_PER_CELL[k] * ncell / world,
+                       "achieved_gbs": gbs, "frac": gbs / peak}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"]) if kern else None
+    roofline = None
+    if dom:
+        roofline = {"bound": "hbm", "kernel": f"stage_tma<{dom[-1]}> x {len(s.ranks)} slabs per step", "achieved": kern[dom]["achieved_gbs"],
+                    "peak": peak, "unit": "GB/s", "frac": kern[dom]["frac"], "traffic": None, "traffic_source": None,
+                    "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL[dom]}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": job_s * 1e3 / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f32 flux / f64 state", "data": "synthetic",
+        "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": "mixed", "scheme": "PLM-minmod + HLLC + Heun",
+                   "kernel": "tma", "cfl": pr.cfl,
+                   "parallelism": (f"{nslab} z slabs, one per GPU (communication boundaries, NCCL all-reduce for dt)" if world > 1 else
+                                   f"{nslab} z slabs in one process on one GPU, advanced in lock step (communication boundaries)"),
+                   "halo_bytes_per_step": halo_bytes,
+                   "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)", "floor_hits": hits},
+        "hbm_roofline_frac_step": value / world * 200.0 / (peak * 1e9),
+        "roofline": roofline, "kernels": kern, "cpu_baseline": None,
+        "e2e": {"value": ncell * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 40 * ncell, "d2h_bytes_per_step": 40 * ncell,
+                "steps": e2e_steps},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -352,11 +478,16 @@ def main():
     ap.add_argument("--integrator", default="heun", choices=["heun", "vanleer"],
                     help="time integrator (PAPER.md Sec. 3.3); the headline metric is quoted on heun")
     ap.add_argument("--zchunk", type=int, default=0, help="planes per slab of the marching kernels (0 = auto)")
+    ap.add_argument("--slabs", type=int, default=1, help="cut the block into this many z slabs in this process (row f-4)")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
+                    help="what --gpus N > 1 means: N replicas (default, DESIGN.md section 9) or N z slabs of one block")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":
         run_reference(args)
+    elif args.slabs > 1 or (args.decomposition == "slab" and int(os.environ.get("WORLD_SIZE", "1")) > 1):
+        run_slabs(args)
     else:
         run_ours(args)
 

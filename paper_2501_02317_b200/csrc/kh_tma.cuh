@@ -319,7 +319,8 @@ __device__ __forceinline__ void plm_m(f2 qm, f2 q, f2 qp, f2& qL, f2& qR)
 // primitives W^{n+1/2} = prim(U + dt/2 L_1(U)) (a float box written over the consumed raw plane and stored by TMA).
 // MODE 2 (with STAGE 2): its corrector U^{n+1} = U^n + dt L_2(W^{n+1/2}): the plane ring and the halo boxes carry the
 // float_t primitives (no recovery, no fp64 chain), U^n arrives through the U0 ring, is updated in place there and stored.
-template <int STAGE, int MODE = 0, typename ST = double>
+// COMM: the block has communication boundaries in z (a separate instantiation: the undivided block pays nothing for them).
+template <int STAGE, int MODE = 0, typename ST = double, bool COMM = false>
 __global__ void __launch_bounds__(NTHREADS, BLOCKS_PER_SM)
 stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
 {
@@ -822,9 +823,9 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
             mbar_expect_tx(&sm.full_raw[slot], RAW_TX);
             // ghost planes of a communication boundary come from the array the neighbouring block has filled
             // (planes further out than two are loaded for the straight-line code only and never used)
-            if (p < 0 && g.bc[4] == BC_COMM)
+            if (COMM && p < 0 && g.bc[4] == BC_COMM)
                 tma_load4(&sm.raw[slot][0][0][0], &maps.in_glo, i0, j0, max(p + 2, 0), 0, &sm.full_raw[slot]);
-            else if (p >= nz && g.bc[5] == BC_COMM)
+            else if (COMM && p >= nz && g.bc[5] == BC_COMM)
                 tma_load4(&sm.raw[slot][0][0][0], &maps.in_ghi, i0, j0, min(p - nz, 1), 0, &sm.full_raw[slot]);
             else
                 tma_load4(&sm.raw[slot][0][0][0], &maps.in_own, i0, j0, sk, 0, &sm.full_raw[slot]);   // (slot stride follows the type)
@@ -834,8 +835,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
         // stage kernel (no separate pack / send / unpack pass, no extra read of the state).
         auto store_plane = [&](int p, const void* src) {
             tma_store4(&maps.out_own, i0, j0, p, 0, src);
-            if (g.bc[4] == BC_COMM && p < 2) tma_store4(&maps.out_plo, i0, j0, p, 0, src);
-            if (g.bc[5] == BC_COMM && p >= nz - 2) tma_store4(&maps.out_phi, i0, j0, p - (nz - 2), 0, src);
+            if (COMM && g.bc[4] == BC_COMM && p < 2) tma_store4(&maps.out_plo, i0, j0, p, 0, src);
+            if (COMM && g.bc[5] == BC_COMM && p >= nz - 2) tma_store4(&maps.out_phi, i0, j0, p - (nz - 2), 0, src);
             tma_commit();
         };
         auto load_halo = [&](int p, int slot) {  // p in [kbeg, kend): an interior plane
@@ -1101,6 +1102,10 @@ inline void configure()
     cudaFuncSetAttribute(stage_tma<1, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_tma<1, 0, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1>) + 128);
+    cudaFuncSetAttribute(stage_tma<2, 0, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2>) + 128);
+    cudaFuncSetAttribute(stage_tma<1, 0, double, true>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_tma<2, 0, double, true>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(stage_tma<1, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<1, 0, float>) + 128);
     cudaFuncSetAttribute(stage_tma<2, 0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<2, 0, float>) + 128);
     cudaFuncSetAttribute(stage_tma<1, 0, float>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
@@ -1110,8 +1115,11 @@ inline void configure()
 inline void launch_stage(int stage, const StageMaps& sm, const Grid& g, Ctrl* ctrl, int zchunk, cudaStream_t stream)
 {
     dim3 grid(g.n[0] / PTX, g.n[1] / PTY, (g.n[2] + zchunk - 1) / zchunk);
-    if (stage == 1) stage_tma<1><<<grid, NTHREADS, sizeof(Smem<1>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
-    else            stage_tma<2><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
+    const bool comm = g.bc[4] == BC_COMM || g.bc[5] == BC_COMM;
+    if (comm && stage == 1) stage_tma<1, 0, double, true><<<grid, NTHREADS, sizeof(Smem<1>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
+    else if (comm)          stage_tma<2, 0, double, true><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
+    else if (stage == 1)    stage_tma<1><<<grid, NTHREADS, sizeof(Smem<1>) + 128, stream>>>(sm.s1, g, ctrl, zchunk);
+    else                    stage_tma<2><<<grid, NTHREADS, sizeof(Smem<2>) + 128, stream>>>(sm.s2, g, ctrl, zchunk);
 }
 
 }  // namespace tma
