@@ -16,8 +16,8 @@
 //     into a ring of NRING slots, completing on the warp's own mbarriers; at the domain edge two extra 2-column boxes
 //     bring the ghost columns from where the boundary rule of Sec. 3.1.1 takes them (periodic wrap,
 //     clamp, mirror), and ghost rows are a choice of box coordinates, exactly as in kh_tma.cuh;
-//   * the update is fp64: raw state from the ring + flux sums, Heun average with U0 (plain
-//     coalesced loads issued one trip ahead), coalesced 8-byte stores; stage 2 reduces the CFL rate of the new state
+//   * the update is fp64: raw state from the ring + flux sums, Heun average with U0 (cp.async
+//     copies of the lane's own column, issued one trip ahead), coalesced 8-byte stores; stage 2 reduces the CFL rate of the new state
 //     (PAPER.md:173).
 // Warps are independent, so their load, convert, solve and update phases interleave on the SM by themselves; 12 warps
 // per SM (three blocks of four warps).
@@ -54,6 +54,8 @@ constexpr unsigned HBOX_BYTES = 5 * 2 * 2 * 8;   // 160
 struct WarpSmem {
     alignas(128) double raw[NRING][5][2][32];    // TMA box of a row pair: [field][row][column]
     alignas(128) double hx[NRING][2][32];        // ghost-column boxes [side][5 fields x 2 rows x 2 columns], padded to 256 B
+    alignas(16) double u0[5][2][32];             // stage 2: U0 of the two rows the NEXT trip updates; every lane copies and reads
+                                                 // its own column only (cp.async), so the slot needs no second buffer
     unsigned long long full[NRING];
 };
 
@@ -196,6 +198,22 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
     const long long col_off = (long long)(owner ? c : 0);
     // ring slots of the pairs p-1 (row 2p-1 updated), p+1 (converted) and p+3 (issued) at trip p; pair p sits in s_upd + 1
     int s_upd = 0, s_conv = 2, s_issue = 4;
+    // U0 of rows 2p-1 and 2p (the rows trip p updates), fetched one trip ahead: 8-byte cp.async copies of the lane's own
+    // column into its own entries of sm.u0, a whole trip of latency hidden (the plain loads of the first version, issued and
+    // consumed in the same trip, cost stage 2 two stalled cycles per issued one: profiles/r2a_strip_full.md, long_sb)
+    auto fetch_u0 = [&](int p) {
+        if (STAGE != 2) return;
+        const bool a = (p > pbeg) && owner, b = (p < pend) && owner;
+        const long long cell = (long long)(2 * p - 1) * nx + col_off;
+        double* d = &sm.u0[0][0][lane];
+#pragma unroll
+        for (int f = 0; f < 5; f++) {
+            if (a) __pipeline_memcpy_async(d + f * 64, U0 + f * N + cell, 8);
+            if (b) __pipeline_memcpy_async(d + f * 64 + 32, U0 + f * N + cell + nx, 8);
+        }
+        __pipeline_commit();
+    };
+    fetch_u0(pbeg);
 
     // Trip p solves the faces of pair p; that completes row 2p-1 (the face above it was missing) and row 2p, which are
     // updated and stored; row 2p+1 waits for the next trip.  The first trip of a slab stores row 2p only, the last one
@@ -227,13 +245,14 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
             tma::to_normal<1>(qRy, R[1]);
         }
         tma::hllc2n<2>(L, R, gas, Fn);
-        // U0 of the two rows for the Heun average: issued here, where the registers of the solver are free again; the
-        // other warps of the SM cover its latency
+        // U0 of the two rows for the Heun average (fetched during the previous trip); the next trip's fetch follows at once
         double2 v0[5];
         if (STAGE == 2) {
+            __pipeline_wait_prior(0);
+            const double* d = &sm.u0[0][0][lane];
 #pragma unroll
-            for (int f = 0; f < 5; f++)
-                v0[f] = make_double2(upd_a ? U0[f * N + cell_a] : 0.0, upd_b ? U0[f * N + cell_a + nx] : 0.0);
+            for (int f = 0; f < 5; f++) v0[f] = make_double2(d[f * 64], d[f * 64 + 32]);   // (rows not updated: stale, unused)
+            if (p + 1 <= pend) fetch_u0(p + 1);
         }
         double ua[5], ub[5];   // new state of rows 2p-1, 2p
         {
