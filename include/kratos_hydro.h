@@ -173,7 +173,9 @@ KRATOS_API int kratos_hydro_status(kratos_hydro_t *h);
 KRATOS_API int kratos_hydro_launch_count(kratos_hydro_t *h, long long *n);
 
 /* Per-kernel timing with CUDA events on the handle's stream.  enable != 0 switches event
- * recording on for step / run; kratos_hydro_get_timing then returns, since the last call to
+ * recording on for step / run: around every launch (enable = 1), or around the launches of every
+ * enable-th step only (enable > 1: two event records cost about 2.5 us of stream time each, which
+ * shows on grids whose step takes a fraction of a millisecond); kratos_hydro_get_timing then returns, since the last call to
  * set_profiling, the summed duration [ms] and launch count of: slot 0 stage-1 kernel,
  * slot 1 stage-2 kernel, slot 2 all other kernels (dt bookkeeping, reductions).
  * ms, launches: host arrays of 3.  Synchronises. */

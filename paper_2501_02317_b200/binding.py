@@ -275,7 +275,8 @@ class KratosHydro:
         return n.value
 
     def set_profiling(self, enable=True):
-        _check(self._L.kratos_hydro_set_profiling(self._h, 1 if enable else 0))
+        """True / 1: events around every launch; n > 1: around the launches of every n-th step; False / 0: off."""
+        _check(self._L.kratos_hydro_set_profiling(self._h, int(enable)))
 
     def get_timing(self):
         """{'stage1': (ms, launches), 'stage2': ..., 'other': ...} since set_profiling."""

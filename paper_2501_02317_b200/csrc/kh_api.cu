@@ -75,8 +75,11 @@ struct kratos_hydro {
     bool rate_valid;  // ctrl->rate_bits holds the rate maximum of U0
     bool pref_valid;  // ctrl->p_ref was computed from the state last given to set_state
     long long launches;
-    // profiling
+    // profiling: event pairs around the launches of every prof_every-th step (prof_on: this step is one of them)
     bool profiling;
+    int prof_every;
+    long long prof_step;
+    bool prof_on;
     std::vector<cudaEvent_t> ev_pool;
     std::vector<std::pair<int, int>> ev_used;  // (slot, index of start event; stop = +1)
     size_t ev_next;
@@ -109,7 +112,7 @@ struct LaunchTimer {
     LaunchTimer(kratos_hydro* h_, int slot_) : h(h_), slot(slot_), idx(-1)
     {
         h->launches++;
-        if (!h->profiling) return;
+        if (!h->profiling || !h->prof_on) return;
         if (h->ev_next + 2 > h->ev_pool.size()) {
             if (h->ev_pool.size() >= 200000) return;  // stop recording, keep running
             for (int i = 0; i < 2; i++) {
@@ -129,6 +132,12 @@ struct LaunchTimer {
         h->ev_used.push_back({slot, idx});
     }
 };
+
+// called once per step before its launches
+void next_step_profiling(kratos_hydro* h)
+{
+    h->prof_on = !h->profiling || (h->prof_step++ % h->prof_every) == 0;
+}
 
 void collect_timing(kratos_hydro* h)
 {
@@ -392,6 +401,9 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
     h->pref_valid = false;
     h->launches = 0;
     h->profiling = false;
+    h->prof_every = 1;
+    h->prof_step = 0;
+    h->prof_on = true;
     h->ev_next = 0;
     for (int s = 0; s < 3; s++) { h->prof_ms[s] = 0; h->prof_n[s] = 0; }
     h->U0 = h->U1 = nullptr;
@@ -590,6 +602,7 @@ int kratos_hydro_step(kratos_hydro_t* h, double dt)
     int rc;
     // first step after set_state: the reference pressure of the mixed-precision kernels comes from this state
     if (!h->pref_valid && h->prec == KRATOS_PREC_MIXED && (rc = launch_cfl_rate(h))) return rc;
+    next_step_profiling(h);
     {
         LaunchTimer lt(h, SLOT_OTHER);
         set_dt_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, dt);
@@ -621,6 +634,7 @@ static int run_impl(kratos_hydro_t* h, double cfl, double t_end, int max_steps, 
     while (done < max_steps) {
         const int nb = (max_steps - done < batch) ? max_steps - done : batch;
         for (int s = 0; s < nb; s++) {
+            next_step_profiling(h);
             {
                 LaunchTimer lt(h, SLOT_OTHER);
                 prepare_step_kernel<<<1, 1, 0, h->stream>>>(h->ctrl);
@@ -724,6 +738,9 @@ int kratos_hydro_set_profiling(kratos_hydro_t* h, int enable)
     h->ev_next = 0;
     for (int s = 0; s < 3; s++) { h->prof_ms[s] = 0; h->prof_n[s] = 0; }
     h->profiling = enable != 0;
+    h->prof_every = enable > 1 ? enable : 1;
+    h->prof_step = 0;
+    h->prof_on = true;
     return KRATOS_OK;
 }
 
@@ -851,6 +868,7 @@ int kratos_hydro_substep(kratos_hydro_t* h, int phase)
     int rc;
     if (phase == KRATOS_PHASE_PREPARE) {
         if (!h->rate_valid || !h->pref_valid) return fail(KRATOS_ERR_ARG, "substep before kratos_hydro_begin_run");
+        next_step_profiling(h);
         LaunchTimer lt(h, SLOT_OTHER);
         prepare_step_kernel<<<1, 1, 0, h->stream>>>(h->ctrl);
         return KRATOS_OK;
