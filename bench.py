@@ -78,7 +78,7 @@ def kernel_name(variant: int, prec: int, stage: int, ndim: int, vanleer: bool = 
     if variant == b.KERNEL_TMA:
         return f"stage_tma<{stage},0,float>" if prec == 2 else f"stage_tma<{stage}>"
     if variant == b.KERNEL_STRIP:
-        return f"stage_strip<{stage}>"
+        return f"stage_strip<{stage},float>" if prec == 2 else f"stage_strip<{stage}>"
     if variant == b.KERNEL_PAIRED:
         return f"stage_pair<{stage},{ndim}>"
     if variant == b.KERNEL_TILED:

@@ -95,7 +95,7 @@ typedef struct kratos_hydro kratos_hydro_t; /* opaque */
                                   tile, halo and U0 planes onto mbarriers and stores each updated plane): mixed
                                   precision, three active axes, nx % 32 == 0, ny % 16 == 0 */
 
-#define KRATOS_KERNEL_STRIP 6  /* 2D blocks (nz = 1, nx and ny even), mixed precision, Heun: one warp per 28-column strip
+#define KRATOS_KERNEL_STRIP 6  /* 2D blocks (nz = 1, nx and ny even; all-fp32 mode: nx % 4 == 0), mixed precision or all-fp32, Heun: one warp per 28-column strip
                                   marching along y, x neighbours by warp shuffles, row pairs by per-warp TMA boxes; no
                                   block barriers */
 

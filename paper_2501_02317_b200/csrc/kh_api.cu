@@ -157,7 +157,7 @@ int auto_variant(const kratos_hydro* h)
     if (h->comm[0] || h->comm[1]) return KRATOS_KERNEL_TMA;   // checked at create: the only kernel that serves them
     if (h->integ == 1) return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;  // van Leer
     if (h->prec == KRATOS_PREC_SINGLE)   // all-fp32 state: the TMA kernel on float boxes, else the general kernel
-        return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : KRATOS_KERNEL_SIMPLE;
+        return (h->maps && h->maps->ok) ? KRATOS_KERNEL_TMA : ((h->smaps && h->smaps->ok) ? KRATOS_KERNEL_STRIP : KRATOS_KERNEL_SIMPLE);
     if (!h->tiled_ok) return KRATOS_KERNEL_SIMPLE;
     if (h->prec != KRATOS_PREC_MIXED) return KRATOS_KERNEL_TILED;
     if (h->maps && h->maps->ok) return KRATOS_KERNEL_TMA;
@@ -184,7 +184,7 @@ int launch_stage(kratos_hydro* h, int stage)
     if (h->variant == KRATOS_KERNEL_TMA) {
         tma::launch_stage(stage, *h->maps, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_STRIP) {
-        strip::launch_stage(stage, *h->smaps, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
+        strip::launch_stage<double>(stage, *h->smaps, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_PAIRED) {
         pr::launch_stage(stage, Uin, h->U0, Uout, g, h->ctrl, pick_zchunk(h), h->stream);
     } else if (h->variant == KRATOS_KERNEL_TILED) {
@@ -212,6 +212,8 @@ int launch_stage_single(kratos_hydro* h, int stage)
     const int threads = 128;
     const long long blocks = (g.N + threads - 1) / threads;
     if (h->variant == KRATOS_KERNEL_TMA) tma::launch_stage_single(stage, *h->maps, g, h->ctrl, pick_zchunk(h), h->stream);
+    else if (h->variant == KRATOS_KERNEL_STRIP)
+        strip::launch_stage<float>(stage, *h->smaps, A, stage == 1 ? B : const_cast<float*>(A), g, h->ctrl, pick_zchunk(h), h->stream);
     else if (stage == 1) stage_simple<float, 1, float><<<(unsigned)blocks, threads, 0, h->stream>>>(A, A, B, g, h->ctrl);
     else            stage_simple<float, 2, float><<<(unsigned)blocks, threads, 0, h->stream>>>(B, A, const_cast<float*>(A), g, h->ctrl);
     cudaError_t e = cudaGetLastError();
@@ -453,9 +455,13 @@ kratos_hydro_t* kratos_hydro_create(int nx, int ny, int nz, double gamma, int sc
         if (h->maps && integ == 0) tma::build_maps(h->maps, h->U0, h->U1, g);
         if (h->maps && integ == 1) tma::build_maps_vl(h->maps, h->U0, (const float*)h->U1, g);
     }
+    if (prec == KRATOS_PREC_SINGLE && strip::supported_single(g)) {
+        h->smaps = new (std::nothrow) strip::StageMaps;
+        if (h->smaps) strip::build_maps(h->smaps, reinterpret_cast<const float*>(h->U0), reinterpret_cast<const float*>(h->U1), g);
+    }
     if (prec == KRATOS_PREC_MIXED && integ == 0 && strip::supported(g)) {
         h->smaps = new (std::nothrow) strip::StageMaps;
-        if (h->smaps) strip::build_maps(h->smaps, h->U0, h->U1, g);
+        if (h->smaps) strip::build_maps(h->smaps, (const double*)h->U0, (const double*)h->U1, g);
     }
     if (h->comm[0] || h->comm[1]) {
         double* none[2] = {nullptr, nullptr};

@@ -1,5 +1,6 @@
 // kh_strip.cuh -- KRATOS_KERNEL_STRIP: the fused stage kernel of 2D blocks (x and y active, nz == 1) in mixed
-// precision (float_t = fp32, float2_t = fp64): one warp = one independent pipeline.
+// precision (float_t = fp32, float2_t = fp64) and in the all-fp32 "Single" mode (float2_t = fp32,
+// PAPER.md:240; the mode of the paper's 2D performance table): one warp = one independent pipeline.
 //
 // A warp owns a strip of SW = 28 columns and marches along y through a slab of rows, two rows per trip:
 //   * lane l holds column x0 - 2 + l of the strip's 32-column window; the two outer lanes on either side are the
@@ -48,13 +49,20 @@ constexpr int NRING = 5;      // row pairs in flight per warp: p-1 (update), p, 
 #endif
 constexpr int WARPS = KH_STRIP_WARPS;           // warps per block (independent of each other)
 constexpr int BLOCKS_PER_SM = KH_STRIP_BLOCKS;  // 12 warps per SM at <= 168 registers
-constexpr unsigned BOX_BYTES = 5 * 2 * 32 * 8;   // 2560
-constexpr unsigned HBOX_BYTES = 5 * 2 * 2 * 8;   // 160
+constexpr unsigned HBOX_BYTES = 160;   // a ghost-column box: 5 fields x 2 rows x 16 bytes (2 doubles or 4 floats)
 
+// ST = float2_t, the type the conserved state is stored in: double, or float in the all-fp32 "Single" mode.
+// The box of a row pair starts on a 16-byte boundary of global memory (a box of floats starting 8 bytes off one raised
+// "illegal instruction" on sm_100a): doubles x0 - 2, 32 wide; floats x0 - 4, 36 wide, the lane's column two elements in.
+template <typename ST> struct Box { static constexpr int W = 32, OFF = 0; };
+template <> struct Box<float> { static constexpr int W = 36, OFF = 2; };
+
+template <typename ST>
 struct WarpSmem {
-    alignas(128) double raw[NRING][5][2][32];    // TMA box of a row pair: [field][row][column]
-    alignas(128) double hx[NRING][2][32];        // ghost-column boxes [side][5 fields x 2 rows x 2 columns], padded to 256 B
-    alignas(16) double u0[5][2][32];             // stage 2: U0 of the two rows the NEXT trip updates; every lane copies and reads
+    struct alignas(128) Slot { ST v[5][2][Box<ST>::W]; };
+    Slot raw[NRING];                             // TMA box of a row pair: [field][row][column]
+    alignas(128) unsigned char hx[NRING][2][256];  // ghost-column boxes [side]: [5 fields][2 rows][16 bytes], padded to 256 B
+    alignas(16) ST u0[5][2][32];                 // stage 2: U0 of the two rows the NEXT trip updates; every lane copies and reads
                                                  // its own column only (cp.async), so the slot needs no second buffer
     unsigned long long full[NRING];
 };
@@ -83,20 +91,26 @@ __device__ __forceinline__ f2 shfl_down2(f2 v)
 // One Heun stage of a 2D block.  STAGE 1: Uout = Uin + dt L(Uin).  STAGE 2: Uout = 1/2 U0 + 1/2 (Uin +
 // dt L(Uin)) (Uout aliases U0) and the CFL rate maximum of Uout.
 // rows_per_slab is even; a warp handles strip (id % nstrips), slab (id / nstrips).
-template <int STAGE>
+template <int STAGE, typename ST = double>
 __global__ void __launch_bounds__(WARPS * 32, BLOCKS_PER_SM)
-stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, Grid g, Ctrl* ctrl, int rows_per_slab,
+stage_strip(const __grid_constant__ Maps maps, const ST* U0, ST* Uout, Grid g, Ctrl* ctrl, int rows_per_slab,
             int nstrips, int nwork)
 {
+    constexpr bool SGL = sizeof(ST) == 4;          // all-fp32 state: float boxes, fp32 recovery and update, no reference pressure
+    constexpr int XW = SGL ? 4 : 2;                // columns of a ghost-column box (16 bytes)
+    constexpr int BW = Box<ST>::W;                 // columns of the row-pair box
+    constexpr int SLOT = sizeof(typename WarpSmem<ST>::Slot) / sizeof(ST);   // element stride of the ring
+    constexpr unsigned BOX_BYTES = 5 * 2 * BW * sizeof(ST);
+    using ST2 = typename std::conditional<SGL, float2, double2>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpSmem& sm = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+    WarpSmem<ST>& sm = reinterpret_cast<WarpSmem<ST>*>(smem_raw)[warp];
 
     const double dt = ctrl->dt;
     if (!(dt > 0.0)) return;  // a step clipped to zero length (run_until past t_end) does nothing
     const int work = blockIdx.x * WARPS + warp;
     if (work >= nwork) return;   // (whole warps: no block-wide synchronisation exists in this kernel)
-    const double pref_d = ctrl->p_ref;
+    const double pref_d = SGL ? 0.0 : ctrl->p_ref;
     const int nx = g.n[0], ny = g.n[1];
     const long long N = g.N;
     const int s = work % nstrips, slab = work / nstrips;
@@ -105,7 +119,8 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
     const int npair = ny / 2;
     const int pbeg = slab * (rows_per_slab / 2);
     const int pend = min(pbeg + rows_per_slab / 2, npair);   // pairs [pbeg, pend)
-    const double gm1 = g.gamma - 1.0;
+    const ST gm1 = ST(g.gamma - 1.0);
+    const ST pref_s = ST(pref_d);
     Gas gas;
     gas.gamma = (float)g.gamma;
     gas.g1 = (float)((g.gamma + 1.0) / (2.0 * g.gamma));
@@ -114,16 +129,16 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
 
     // ---- where this lane's column comes from (Sec. 3.1.1 in x) ----
     // interior column: the strip's own box.  Ghost column (c in {-2,-1} or {nx, nx+1}): one of the two ghost boxes.
-    const HaloSide xlo = halo_side(-2, nx, g.bc[0], g.bc[1]);
-    const HaloSide xhi = halo_side(nx, nx, g.bc[0], g.bc[1]);
+    const HaloSide xlo = halo_side(-2, nx, g.bc[0], g.bc[1], XW);
+    const HaloSide xhi = halo_side(nx, nx, g.bc[0], g.bc[1], XW);
     const bool ghost_lo = c < 0, ghost_hi = c >= nx && c < nx + 2;
     const bool need_lo = x0 - 2 < 0, need_hi = x0 - 2 + 32 > nx;      // warp-uniform: this strip touches a domain edge
     const int rx = ghost_lo ? xlo.rule : (ghost_hi ? xhi.rule : VN_KEEP);
     const int hx_idx = ghost_lo ? ((c == -2) ? xlo.idx0 : xlo.idx1) : ((c == nx) ? xhi.idx0 : xhi.idx1);
     const bool owner = lane >= 2 && lane < 2 + SW && c < nx;          // this lane's cells are written by this warp
     // element offsets of this lane inside a ring slot: own box [field][row][32], ghost box [side][field][row][2]
-    const double* const own_base = &sm.raw[0][0][0][lane];
-    const double* const hx_base = &sm.hx[0][ghost_hi ? 1 : 0][hx_idx];
+    const ST* const own_base = &sm.raw[0].v[0][0][lane + Box<ST>::OFF];
+    const ST* const hx_base = reinterpret_cast<const ST*>(&sm.hx[0][ghost_hi ? 1 : 0][0]) + hx_idx;
     const bool from_ghost_box = ghost_lo || ghost_hi;
 
     if (lane == 0) {
@@ -141,7 +156,7 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
         const int row = (q < 0) ? ylo.start : ((q >= npair) ? yhi.start : 2 * q);
         unsigned long long* bar = &sm.full[slot];
         tma::mbar_expect_tx(bar, tx_bytes);
-        tma_load3(&sm.raw[slot][0][0][0], &maps.in_own, x0 - 2, row, 0, bar);
+        tma_load3(&sm.raw[slot].v[0][0][0], &maps.in_own, x0 - 2 - Box<ST>::OFF, row, 0, bar);
         if (need_lo) tma_load3(&sm.hx[slot][0][0], &maps.in_cols, xlo.start, row, 0, bar);
         if (need_hi) tma_load3(&sm.hx[slot][1][0], &maps.in_cols, xhi.start, row, 0, bar);
     };
@@ -154,19 +169,19 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
         else if (q >= npair) { i0 = yhi.idx0; i1 = yhi.idx1; ry = yhi.rule; }
         tma::mbar_wait_parity(&sm.full[slot], (phase_bits >> slot) & 1u);
         phase_bits ^= 1u << slot;
-        double ua[5], ub[5];
+        ST ua[5], ub[5];
         if (from_ghost_box) {
-            const double* b = hx_base + slot * (2 * 32);
+            const ST* b = hx_base + slot * (2 * 256 / (int)sizeof(ST));
 #pragma unroll
-            for (int f = 0; f < 5; f++) { ua[f] = b[f * 4 + i0 * 2]; ub[f] = b[f * 4 + i1 * 2]; }
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 2 * XW + i0 * XW]; ub[f] = b[f * 2 * XW + i1 * XW]; }
         } else {
-            const double* b = own_base + slot * (5 * 2 * 32);
+            const ST* b = own_base + slot * SLOT;
 #pragma unroll
-            for (int f = 0; f < 5; f++) { ua[f] = b[f * 64 + i0 * 32]; ub[f] = b[f * 64 + i1 * 32]; }
+            for (int f = 0; f < 5; f++) { ua[f] = b[f * 2 * BW + i0 * BW]; ub[f] = b[f * 2 * BW + i1 * BW]; }
         }
         float Wa[5], Wb[5];
-        const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_d, rx, ry, VN_KEEP, Wa);
-        const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_d, rx, ry, VN_KEEP, Wb);
+        const int ha = recover(ua[0], ua[1], ua[2], ua[3], ua[4], gm1, pref_s, rx, ry, VN_KEEP, Wa);
+        const int hb = recover(ub[0], ub[1], ub[2], ub[3], ub[4], gm1, pref_s, rx, ry, VN_KEEP, Wb);
         if (count && owner) hits += ha + hb;
 #pragma unroll
         for (int f = 0; f < 5; f++) W[f] = mk(Wa[f], Wb[f]);
@@ -178,7 +193,7 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
     f2 WA[5], WB[5];              // W(p) and W(p+1), swapping roles from trip to trip
     float Wmy[5];                 // upper row of pair p-1
     float QLc[5];                 // left state of the y face below row 2p (limited state of row 2p-1 at its upper face)
-    double pend_y[5];             // flux sum of row 2p-1, lacking the face above it (which trip p solves)
+    ST pend_y[5];                 // flux sum of row 2p-1, lacking the face above it (which trip p solves)
     {
         f2 Wm[5];
         convert(pbeg - 1, 0, Wm, false);
@@ -189,10 +204,10 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
             plm(mk(Wm[f].x, Wm[f].x), Wm[f], mk(Wm[f].y, WA[f].x), qL, qR);   // row 2pbeg-1 from rows 2pbeg-2, 2pbeg-1, 2pbeg
             QLc[f] = qL.y;
             Wmy[f] = Wm[f].y;
-            pend_y[f] = 0.0;
+            pend_y[f] = ST(0);
         }
     }
-    const double dtdx = dt * g.inv_dx[0], dtdy = dt * g.inv_dx[1];
+    const ST dtdx = ST(dt * g.inv_dx[0]), dtdy = ST(dt * g.inv_dx[1]);
     const CflConst<float> cc(g);
     f2 rate = mk(0.0f, 0.0f);
     const long long col_off = (long long)(owner ? c : 0);
@@ -205,11 +220,11 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
         if (STAGE != 2) return;
         const bool a = (p > pbeg) && owner, b = (p < pend) && owner;
         const long long cell = (long long)(2 * p - 1) * nx + col_off;
-        double* d = &sm.u0[0][0][lane];
+        ST* d = &sm.u0[0][0][lane];
 #pragma unroll
         for (int f = 0; f < 5; f++) {
-            if (a) __pipeline_memcpy_async(d + f * 64, U0 + f * N + cell, 8);
-            if (b) __pipeline_memcpy_async(d + f * 64 + 32, U0 + f * N + cell + nx, 8);
+            if (a) __pipeline_memcpy_async(d + f * 64, U0 + f * N + cell, sizeof(ST));
+            if (b) __pipeline_memcpy_async(d + f * 64 + 32, U0 + f * N + cell + nx, sizeof(ST));
         }
         __pipeline_commit();
     };
@@ -246,34 +261,33 @@ stage_strip(const __grid_constant__ Maps maps, const double* U0, double* Uout, G
         }
         tma::hllc2n<2>(L, R, gas, Fn);
         // U0 of the two rows for the Heun average (fetched during the previous trip); the next trip's fetch follows at once
-        double2 v0[5];
+        ST2 v0[5];
         if (STAGE == 2) {
             __pipeline_wait_prior(0);
-            const double* d = &sm.u0[0][0][lane];
+            const ST* d = &sm.u0[0][0][lane];
 #pragma unroll
-            for (int f = 0; f < 5; f++) v0[f] = make_double2(d[f * 64], d[f * 64 + 32]);   // (rows not updated: stale, unused)
+            for (int f = 0; f < 5; f++) { v0[f].x = d[f * 64]; v0[f].y = d[f * 64 + 32]; }   // (rows not updated: stale, unused)
             if (p + 1 <= pend) fetch_u0(p + 1);
         }
-        double ua[5], ub[5];   // new state of rows 2p-1, 2p
+        ST ua[5], ub[5];   // new state of rows 2p-1, 2p
         {
             f2 Fx[5], Fy[5];
             tma::from_normal<0>(Fn[0], Fx);
             tma::from_normal<1>(Fn[1], Fy);
-            const double* ba = own_base + s_upd * (5 * 2 * 32) + 32;                               // row 2p-1 in the ring
-            const double* bb = own_base + ((s_upd + 1 == NRING) ? 0 : s_upd + 1) * (5 * 2 * 32);   // row 2p
+            const ST* ba = own_base + s_upd * SLOT + BW;                                       // row 2p-1 in the ring
+            const ST* bb = own_base + ((s_upd + 1 == NRING) ? 0 : s_upd + 1) * SLOT;   // row 2p
 #pragma unroll
             for (int f = 0; f < 5; f++) {
                 const f2 fxh = shfl_down2(Fx[f]);                          // flux through the face at c + 1/2
-                const double flo = (double)Fy[f].x, fin = (double)Fy[f].y;
+                const ST flo = (ST)Fy[f].x, fin = (ST)Fy[f].y;
                 // fp64 update.  Row 2p-1: its sum so far and the face above it (2p-1/2).
                 // Row 2p: x faces, y faces 2p-1/2 (+) and 2p+1/2 (-).  Row 2p+1 so far: x faces, y face 2p+1/2 (+).
-                double xa = __dadd_rn(ba[f * 64], __fma_rn(-dtdy, flo, pend_y[f]));
-                double xb = __dadd_rn(bb[f * 64], __fma_rn(dtdy, __dadd_rn(flo, -fin),
-                                                           __dmul_rn(dtdx, __dadd_rn((double)Fx[f].x, -(double)fxh.x))));
-                pend_y[f] = __fma_rn(dtdy, fin, __dmul_rn(dtdx, __dadd_rn((double)Fx[f].y, -(double)fxh.y)));
+                ST xa = add_(ba[f * 2 * BW], fma_(-dtdy, flo, pend_y[f]));
+                ST xb = add_(bb[f * 2 * BW], fma_(dtdy, sub_(flo, fin), mul_(dtdx, sub_((ST)Fx[f].x, (ST)fxh.x))));
+                pend_y[f] = fma_(dtdy, fin, mul_(dtdx, sub_((ST)Fx[f].y, (ST)fxh.y)));
                 if (STAGE == 2) {
-                    xa = __fma_rn(0.5, v0[f].x, __dmul_rn(0.5, xa));
-                    xb = __fma_rn(0.5, v0[f].y, __dmul_rn(0.5, xb));
+                    xa = fma_(ST(0.5), v0[f].x, mul_(ST(0.5), xa));
+                    xb = fma_(ST(0.5), v0[f].y, mul_(ST(0.5), xb));
                 }
                 ua[f] = xa;
                 ub[f] = xb;
@@ -329,17 +343,21 @@ inline bool supported(const Grid& g)
     return g.active[0] && g.active[1] && !g.active[2] && g.n[0] % 2 == 0 && g.n[1] % 2 == 0 && g.n[0] >= 4 && g.n[1] >= 4;
 }
 
-// Tensor map over the 2D state U[5][ny][nx] (fp64, x fastest) with a box of bx x 2 x 5.
-inline bool make_map(CUtensorMap* m, const double* U, const Grid& g, int bx)
+// all-fp32 "Single" mode: float boxes need 16-byte row strides
+inline bool supported_single(const Grid& g) { return supported(g) && g.n[0] % 4 == 0; }
+
+// Tensor map over the 2D state U[5][ny][nx] (x fastest; doubles or floats) with a box of bx x 2 x 5.
+template <typename ST>
+inline bool make_map(CUtensorMap* m, const ST* U, const Grid& g, int bx)
 {
     tma::EncodeTiledFn fn = tma::encode_tiled_fn();
     if (!fn) return false;
     const cuuint64_t dims[3] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], 5};
-    const cuuint64_t strides[2] = {(cuuint64_t)g.n[0] * 8, (cuuint64_t)g.N * 8};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.n[0] * sizeof(ST), (cuuint64_t)g.N * sizeof(ST)};
     const cuuint32_t box[3] = {(cuuint32_t)bx, 2, 5};
     const cuuint32_t estr[3] = {1, 1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+    return fn(m, sizeof(ST) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)U, dims, strides, box,
+              estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -348,12 +366,15 @@ struct StageMaps {
     bool ok;
 };
 
-inline void build_maps(StageMaps* sm, const double* A, const double* B, const Grid& g)
+// ghost-column boxes are 16 bytes wide: 2 doubles or 4 floats
+template <typename ST>
+inline void build_maps(StageMaps* sm, const ST* A, const ST* B, const Grid& g)
 {
     sm->ok = false;
-    if (!supported(g)) return;
-    if (!make_map(&sm->s1.in_own, A, g, 32) || !make_map(&sm->s1.in_cols, A, g, 2) ||
-        !make_map(&sm->s2.in_own, B, g, 32) || !make_map(&sm->s2.in_cols, B, g, 2))
+    if (sizeof(ST) == 4 ? !supported_single(g) : !supported(g)) return;
+    const int xw = 16 / (int)sizeof(ST);
+    if (!make_map(&sm->s1.in_own, A, g, Box<ST>::W) || !make_map(&sm->s1.in_cols, A, g, xw) ||
+        !make_map(&sm->s2.in_own, B, g, Box<ST>::W) || !make_map(&sm->s2.in_cols, B, g, xw))
         return;
     sm->ok = true;
 }
@@ -374,15 +395,22 @@ inline int auto_rows(const Grid& g)
     return rows < g.n[1] ? rows : g.n[1];
 }
 
+template <typename ST>
+inline void configure_for()
+{
+    cudaFuncSetAttribute(stage_strip<1, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem<ST>)));
+    cudaFuncSetAttribute(stage_strip<2, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem<ST>)));
+    cudaFuncSetAttribute(stage_strip<1, ST>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(stage_strip<2, ST>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
 inline void configure()
 {
-    cudaFuncSetAttribute(stage_strip<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem)));
-    cudaFuncSetAttribute(stage_strip<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS * sizeof(WarpSmem)));
-    cudaFuncSetAttribute(stage_strip<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(stage_strip<2>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    configure_for<double>();
+    configure_for<float>();
 }
 
-inline void launch_stage(int stage, const StageMaps& sm, const double* U0, double* Uout, const Grid& g, Ctrl* ctrl, int rows,
+template <typename ST>
+inline void launch_stage(int stage, const StageMaps& sm, const ST* U0, ST* Uout, const Grid& g, Ctrl* ctrl, int rows,
                          cudaStream_t stream)
 {
     rows = (rows + 1) & ~1;
@@ -390,9 +418,9 @@ inline void launch_stage(int stage, const StageMaps& sm, const double* U0, doubl
     const int nslabs = (g.n[1] + rows - 1) / rows;
     const int nwork = nstrips * nslabs;
     const unsigned blocks = (unsigned)((nwork + WARPS - 1) / WARPS);
-    const size_t smem = WARPS * sizeof(WarpSmem);
-    if (stage == 1) stage_strip<1><<<blocks, WARPS * 32, smem, stream>>>(sm.s1, U0, Uout, g, ctrl, rows, nstrips, nwork);
-    else            stage_strip<2><<<blocks, WARPS * 32, smem, stream>>>(sm.s2, U0, Uout, g, ctrl, rows, nstrips, nwork);
+    const size_t smem = WARPS * sizeof(WarpSmem<ST>);
+    if (stage == 1) stage_strip<1, ST><<<blocks, WARPS * 32, smem, stream>>>(sm.s1, U0, Uout, g, ctrl, rows, nstrips, nwork);
+    else            stage_strip<2, ST><<<blocks, WARPS * 32, smem, stream>>>(sm.s2, U0, Uout, g, ctrl, rows, nstrips, nwork);
 }
 
 }  // namespace strip

@@ -749,7 +749,8 @@ from parity_utils import assert_parity_single  # noqa: E402
 SINGLE = binding.PREC_SINGLE
 CASES_SINGLE = [((45, 19, 23), (P, P, P, P, P, P)), ((64, 32, 10), (F, F, O, O, R, R)), ((96, 48, 12), (R, O, P, P, F, R)),
                 ((37, 21, 1), (P, P, P, P, P, P)), ((64, 48, 1), (R, R, O, F, P, P)), ((100, 38, 1), (P, P, F, R, P, P)),
-                ((50, 1, 1), (F, F, P, P, P, P)), ((1, 20, 22), (P, P, R, R, P, P))]
+                ((50, 1, 1), (F, F, P, P, P, P)), ((1, 20, 22), (P, P, R, R, P, P)),
+                ((60, 34, 1), (F, O, R, R, P, P)), ((128, 96, 1), (P, P, P, P, P, P))]   # 2D, nx % 4 == 0: the strip kernel on float boxes
 
 
 def r32(U):
@@ -812,3 +813,25 @@ def test_single_mode_run_conservation_and_fixed_point():
     h.destroy()
     with pytest.raises(Exception):   # the van Leer integrator is not offered with an fp32 state
         binding.KratosHydro(40, 20, 12, 1.5, (P,) * 6, precision=SINGLE, integrator=VL)
+
+
+@pytest.mark.parametrize("rows", [2, 6, 10, 1000])
+def test_single_mode_strip_kernel_is_chosen_and_its_slab_seams_are_invisible(rows):
+    """2D blocks with nx % 4 == 0 run the Single mode on the strip kernel (float boxes); the height of the slabs the warps
+    march through must not change a bit of the result."""
+    pr = inputs.random_smooth(84, 40, 1, seed=9, gamma=1.4, bc=(P, P, R, O, P, P))
+    U = r32(pr.U)
+    out = []
+    for r in (0, rows):
+        h = binding.KratosHydro(84, 40, 1, pr.gamma, pr.bc, precision=SINGLE)
+        assert h.get_kernel() == binding.KERNEL_STRIP
+        if r:
+            h.set_zchunk(r)
+        h.set_state(U)
+        h.run(0.4, 5)
+        out.append(h.get_state())
+        h.destroy()
+    np.testing.assert_array_equal(out[0], out[1])
+    h = binding.KratosHydro(86, 40, 1, pr.gamma, pr.bc, precision=SINGLE)    # nx % 4 != 0: the general kernel
+    assert h.get_kernel() == SIMPLE
+    h.destroy()
