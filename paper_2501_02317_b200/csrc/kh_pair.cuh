@@ -168,11 +168,7 @@ __device__ __forceinline__ int recover(double rho, double mx, double my, double 
     // (m.m)/rho with m.m formed first: it does not wait for the reciprocal, which shortens the dependent chain
     const double m2 = __dmul_rn(__fma_rn(mz, mz, __fma_rn(my, my, __dmul_rn(mx, mx))), ir);
     double p = __dmul_rn(gm1, __fma_rn(-0.5, m2, e));
-#ifdef KH_NO_PREF_FLOOR
-    const double pfl = KH_P_FLOOR;
-#else
     const double pfl = fmax(KH_P_FLOOR, __dmul_rn(pref, 0x1p-22));
-#endif
     const bool lo_p = p < pfl;
     p = lo_p ? pfl : p;
     if (rx | ry | rz) {

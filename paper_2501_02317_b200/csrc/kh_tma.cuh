@@ -154,11 +154,7 @@ __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commi
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-#ifdef KH_WHATIF_NOBAR   // timing experiment only (wrong results): how much do the block barriers cost?
-__device__ __forceinline__ void block_bar() { __syncwarp(); }
-#else
 __device__ __forceinline__ void block_bar() { asm volatile("bar.sync 0;" ::: "memory"); }
-#endif
 
 // Stored pressure deviation of a float_t primitive (van Leer corrector): p - pref with the same two-ulp floor as
 // pr::recover, so that the pressure rebuilt by the Riemann solver stays > 0.
@@ -193,11 +189,7 @@ __device__ __forceinline__ HaloSide halo_side(int c0, int n, int bc_lo, int bc_h
 // three packed multiplications instead of two more MUFU operations per face pair (the XU pipe, which also carries the
 // fp32 <-> fp64 conversions, is the busiest one of this kernel).  A few ulp of error in a factor that only enters
 // through max(p*/p_K - 1, 0).
-#ifndef KH_RCP_MUFU
 #define KH_RCP_P(p, rho, t) mul2(mul2(bc(g.gamma), rho), mul2(t, t))
-#else
-#define KH_RCP_P(p, rho, t) rcp2(p)
-#endif
 template <int N>
 __device__ __forceinline__ void hllc2n(const f2 (&L)[N][5], const f2 (&R)[N][5], const Gas& g, f2 (&F)[N][5])
 {
