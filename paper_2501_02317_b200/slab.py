@@ -223,8 +223,18 @@ class SlabSolver:
     def set_state(self, U):
         """U: the state of the WHOLE block, [5, nz, ny, nx] float64 on the host (every rank takes its planes), or
         {rank: local state} for the ranks this process owns."""
-        for r, b in self.blocks.items():
-            b.set_state(U[r] if isinstance(U, dict) else self.dec.scatter(U, r))
+        import torch
+        if isinstance(U, torch.Tensor):
+            # a torch tensor (pinned host memory or device): one copy onto the device, the slabs are cut there
+            with self._ctx():
+                Ud = U.to(self.device, non_blocking=True).reshape(5, self.shape[2], self.shape[1], self.shape[0])
+                for r, b in self.blocks.items():
+                    z0, z1 = self.dec.planes(r)
+                    b.set_state(Ud[:, z0:z1].contiguous())
+                del Ud
+        else:
+            for r, b in self.blocks.items():
+                b.set_state(U[r] if isinstance(U, dict) else self.dec.scatter(U, r))
         # one reference pressure for the whole domain (reading S17): the smallest of the blocks' own choices
         p = min(b.get_reference_pressure() for b in self.blocks.values())
         p = self.comm.all_min_float(p)
@@ -239,6 +249,22 @@ class SlabSolver:
     def get_state(self):
         """{rank: local state} of the ranks this process owns."""
         return {r: b.get_state() for r, b in self.blocks.items()}
+
+    def get_state_into(self, out):
+        """Local mode: the whole block into ``out``, a float64 torch tensor of 5*nx*ny*nz elements (pinned host memory or
+        device); the slabs are joined on the device and leave in one copy."""
+        import torch
+        nx, ny, nz = self.shape
+        with self._ctx():
+            full = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=self.device)
+            for r, b in self.blocks.items():
+                z0, z1 = self.dec.planes(r)
+                part = torch.empty((5, z1 - z0, ny, nx), dtype=torch.float64, device=self.device)
+                b.get_state(part)
+                full[:, z0:z1] = part
+            out.view(5, nz, ny, nx).copy_(full, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        return out
 
     def get_state_global(self):
         """The whole block on every rank (host).  Local mode: a gather; distributed: an all-gather of the slabs."""

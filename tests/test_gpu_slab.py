@@ -134,3 +134,22 @@ def test_substeps_equal_run_on_a_block_without_cuts():
         out.append((t, h.get_state()))
         h.destroy()
     assert out[0][0] == out[1][0] and np.array_equal(out[0][1], out[1][1])
+
+
+def test_state_through_torch_tensors():
+    """set_state from a pinned host tensor (one H2D copy, slabs cut on the device) and get_state_into (slabs joined on the
+    device, one D2H copy) move exactly the bytes the numpy path moves."""
+    import torch
+    nx, ny, nz = 64, 32, 18
+    pr = inputs.random_smooth(nx, ny, nz, seed=4, bc=(P,) * 6, gamma=1.4)
+    s = SlabSolver(nx, ny, nz, pr.gamma, pr.bc, world=3)
+    host = torch.from_numpy(pr.U.copy()).pin_memory()
+    s.set_state(host)
+    out = torch.empty_like(host).pin_memory()
+    s.get_state_into(out)
+    assert np.array_equal(out.numpy(), pr.U)
+    s.run(pr.cfl, 2)
+    a = s.get_state_global()
+    s.get_state_into(out)
+    assert np.array_equal(out.numpy(), a)
+    s.destroy()
