@@ -116,36 +116,50 @@ class _LocalComm:
 
 
 class _DistComm:
-    """One process per GPU (torch.distributed, NCCL on GPUs; gloo for the CPU test of the host logic)."""
+    """One process per GPU (torch.distributed).  NCCL: the collectives are enqueued on the current CUDA stream, so they
+    order the ranks' streams without a host round trip.  Any other backend (gloo: the CPU test of the host logic, and two
+    processes sharing the one GPU of a test box): the stream is drained first and the collective runs on host tensors."""
 
     def __init__(self, group=None):
         import torch.distributed as dist
         self.dist, self.group = dist, group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.nccl = dist.get_backend(group) == "nccl"
         self._token = None
 
-    def sync(self, device):
-        # a one-element all-reduce on the current stream: no rank's stream passes it before every rank's has reached it
+    def _drain(self, device):
         import torch
-        if self._token is None or self._token.device != torch.device(device):
-            self._token = torch.zeros(1, dtype=torch.float32, device=device)
+        if not self.nccl and torch.device(device).type == "cuda":
+            torch.cuda.current_stream().synchronize()
+
+    def sync(self, device):
+        # no rank passes this point before every rank's stream has reached it
+        import torch
+        self._drain(device)
+        dev = device if self.nccl else "cpu"
+        if self._token is None or self._token.device != torch.device(dev):
+            self._token = torch.zeros(1, dtype=torch.float32, device=dev)
         self.dist.all_reduce(self._token, group=self.group)
 
     def all_max(self, t):
-        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+        if self.nccl or t.device.type == "cpu":
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+            return t
+        self._drain(t.device)
+        h = t.cpu()
+        self.dist.all_reduce(h, op=self.dist.ReduceOp.MAX, group=self.group)
+        t.copy_(h)
         return t
 
     def all_min_float(self, x):
         import torch
-        dev = "cuda" if self.dist.get_backend(self.group) == "nccl" else "cpu"
-        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+        t = torch.tensor([float(x)], dtype=torch.float64, device="cuda" if self.nccl else "cpu")
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN, group=self.group)
         return float(t.item())
 
     def all_sum(self, a):
         import torch
-        dev = "cuda" if self.dist.get_backend(self.group) == "nccl" else "cpu"
-        t = torch.as_tensor(np.asarray(a, dtype=np.float64), device=dev)
+        t = torch.as_tensor(np.asarray(a, dtype=np.float64), device="cuda" if self.nccl else "cpu")
         self.dist.all_reduce(t, group=self.group)
         return t.cpu().numpy()
 

@@ -153,3 +153,57 @@ def test_state_through_torch_tensors():
     s.get_state_into(out)
     assert np.array_equal(out.numpy(), a)
     s.destroy()
+
+
+# --------------------------------------------------------------------------- one process per slab (the deployment layout)
+def _ipc_worker(rank, world, port, shape, bc, nsteps, out):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)   # (NCCL refuses two ranks on one GPU; the box has one)
+    try:
+        torch.cuda.set_device(0)
+        nx, ny, nz = shape
+        pr = inputs.random_smooth(nx, ny, nz, seed=31, bc=bc, gamma=1.4)
+        s = SlabSolver(nx, ny, nz, pr.gamma, pr.bc)                # distributed: this process owns the slab of its rank
+        assert s.ranks == [rank] and s.world == world
+        s.set_state(pr.U)
+        t = s.run(pr.cfl, nsteps)
+        U = s.get_state_global()
+        out.put((rank, t, U, s.p_ref, s.floor_hits()))
+        dist.barrier()
+        s.destroy()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("shape,bc,world", [((64, 32, 24), (P, P, P, P, P, P), 2), ((32, 32, 21), (F, F, R, R, O, R), 3)])
+def test_one_process_per_slab_through_cuda_ipc(shape, bc, world):
+    """The layout of a multi-GPU run -- one process per slab, the neighbours' ghost arrays mapped through CUDA IPC handles
+    (kratos_hydro_ghost_ipc_handle / open_peer), reductions and ordering through the process group -- on the one GPU of the
+    test box: the processes share it, no kernel waits for another (the host drains the stream before every collective).
+    Bit for bit the undivided block."""
+    import socket
+    import torch.multiprocessing as mp
+    nsteps = 4
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, shape, bc, nsteps, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=300) for _ in range(world)), key=lambda x: x[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    nx, ny, nz = shape
+    pr = inputs.random_smooth(nx, ny, nz, seed=31, bc=bc, gamma=1.4)
+    Uu, tu, _, _, hits_u = undivided(pr, nsteps, res[0][3])
+    for rank, t, U, p_ref, hits in res:
+        assert p_ref == res[0][3] and hits == 0 and hits_u == 0
+        assert t == tu
+        assert np.array_equal(U, Uu)
