@@ -239,7 +239,8 @@ KRATOS_API int kratos_hydro_set_rate(kratos_hydro_t *h, const double *rate, int 
 
 /* Reference pressure of the mixed-precision solver (see the top of this file; 0 in the other modes).  get computes it from
  * the current state if that has not happened yet.  set replaces it (rounded to fp32; >= 0) until the next set_state: blocks
- * of one decomposed domain must share one value (reading S17).  p_ref: host.  Both synchronise. */
+ * of one decomposed domain must share one value (reading S17).  p_ref: host.  get synchronises; set is asynchronous
+ * (stream-ordered like set_state from a device pointer). */
 KRATOS_API int kratos_hydro_get_reference_pressure(kratos_hydro_t *h, double *p_ref);
 KRATOS_API int kratos_hydro_set_reference_pressure(kratos_hydro_t *h, double p_ref);
 

@@ -278,6 +278,8 @@ int launch_cfl_rate(kratos_hydro* h)
     return KRATOS_OK;
 }
 
+__global__ void set_pref_kernel(Ctrl* ctrl, double p_ref) { ctrl->p_ref = p_ref; }
+
 __global__ void configure_run_kernel(Ctrl* ctrl, double cfl, double t_end, double t)
 {
     ctrl->cfl = cfl;
@@ -935,9 +937,12 @@ int kratos_hydro_set_reference_pressure(kratos_hydro_t* h, double p_ref)
     const float m = (float)p_ref;   // the fp64 recovery and the fp32 solver must use the very same number
     if (!(m >= 0.0f) || !(m < 3.0e38f)) return fail(KRATOS_ERR_ARG, "reference pressure must be >= 0 and finite in fp32");
     DeviceGuard dg(h);
-    const double v = (double)m;
-    CUDA_TRY(cudaMemcpyAsync(&h->ctrl->p_ref, &v, sizeof(double), cudaMemcpyHostToDevice, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    {
+        LaunchTimer lt(h, SLOT_OTHER);
+        set_pref_kernel<<<1, 1, 0, h->stream>>>(h->ctrl, (double)m);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "set_reference_pressure: %s", cudaGetErrorString(e));
     h->pref_valid = true;
     return KRATOS_OK;
 }
