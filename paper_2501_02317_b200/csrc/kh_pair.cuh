@@ -70,6 +70,17 @@ __device__ __forceinline__ void plm(f2 qm, f2 q, f2 qp, f2& qL, f2& qR)
     qR = fma2(bc(-0.5f), s, q);
 }
 
+// The same for a pair of cells that are neighbours along the axis (rows 2w, 2w+1 of a column): face states of both from the
+// four values below, q.x, q.y, above.  Operation for operation plm(mk(below, q.x), q, mk(q.y, above), ...): the three undivided
+// differences are formed once, as scalars (the packed form has to assemble two shifted register pairs first: four moves).
+__device__ __forceinline__ void plm_along_pair(float below, f2 q, float above, f2& qL, f2& qR)
+{
+    const float d0 = __fadd_rn(q.x, -below), d1 = __fadd_rn(q.y, -q.x), d2 = __fadd_rn(above, -q.y);
+    const f2 s = mk(minmod(d0, d1), minmod(d1, d2));
+    qL = fma2(bc(0.5f), s, q);
+    qR = fma2(bc(-0.5f), s, q);
+}
+
 struct Gas {
     float gamma, g1, igm1, pref;
 };
@@ -381,7 +392,7 @@ stage_pair(const double* __restrict__ Uin, const double* U0, double* Uout, Grid 
                     qlx[f * QXF + 1] = qL;
                     const f2 below = wt[f * WTF - (PTX + 4)], above = wt[f * WTF + (PTX + 4)];
                     f2 qLy;
-                    plm(mk(below.y, q.x), q, mk(q.y, above.x), qLy, QRy[f]);
+                    plm_along_pair(below.y, q, above.x, qLy, QRy[f]);
                     QLyo[f] = qLy.x;
                     qly[f * QYF + PTX] = qLy.y;
                 }

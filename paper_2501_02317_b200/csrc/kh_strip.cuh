@@ -246,7 +246,7 @@ stage_strip(const __grid_constant__ Maps maps, const ST* U0, ST* Uout, Grid g, C
             for (int f = 0; f < 5; f++) {
                 const f2 xm = shfl_up2(W0[f]), xp = shfl_down2(W0[f]);
                 plm(xm, W0[f], xp, qLx[f], qRx[f]);
-                plm(mk(Wmy[f], W0[f].x), W0[f], mk(W0[f].y, Wp[f].x), qLy[f], qRy[f]);
+                pr::plm_along_pair(Wmy[f], W0[f], Wp[f].x, qLy[f], qRy[f]);
                 Wmy[f] = W0[f].y;
             }
             f2 t[5];

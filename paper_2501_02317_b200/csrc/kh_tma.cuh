@@ -573,7 +573,8 @@ stage_tma(const __grid_constant__ Maps maps, Grid g, Ctrl* ctrl, int zchunk)
                 for (int f = 0; f < 5; f++) {
                     const f2 q = Wb[f];  // W(k+1)
                     plm_m<MODE>(xm[f], q, xp[f], qLx[f], QRx[f]);
-                    plm_m<MODE>(mk(below[f], q.x), q, mk(q.y, above[f]), qLy[f], QRy[f]);
+                    if (MODE == 1) { qLy[f] = q; QRy[f] = q; }
+                    else pr::plm_along_pair(below[f], q, above[f], qLy[f], QRy[f]);
                     QLyo[f] = qLy[f].x;
                 }
                 if (MODE == 1) {
