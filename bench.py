@@ -518,7 +518,7 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64", "single"],
                     help="mixed: fp32 flux / fp64 state (the headline); fp64: all-fp64; single: all-fp32 (PAPER.md:240)")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--e2e-chunk", type=int, default=64, help="planes per chunk of the streamed end-to-end step")
+    ap.add_argument("--e2e-chunk", type=int, default=32, help="planes per chunk of the streamed end-to-end step")
     ap.add_argument("--e2e-serial", action="store_true", help="end-to-end leg: whole block in, step, whole block out")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", default="auto", choices=["auto", "simple", "tiled", "paired", "tma"],

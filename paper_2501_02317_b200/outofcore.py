@@ -7,7 +7,9 @@ x the two-cell stencil of PLM + HLLC), so the block is cu
 travels with four extra planes on either cut side, is advanced as a block of its own (the extra planes absorb what the
 artificial Free boundary at their outer end gets wrong; the domain's real boundary rule is kept where a chunk touches the
 end of the block), and only its own planes travel back.  Two buffers on two streams keep the upload of
-chunk i+1, the kernels of chunk i and the download of chunk i-1 in flight together.  The same scheme steps a block that does
+chunk i+1, the kernels of chunk i and the download of chunk i-1 in flight together; the overlap planes a chunk shares with
+its predecessor are copied on the device, so every plane crosses the bus once per direction and step (a periodic block
+uploads its wrapped overlap a second time).  The same scheme steps a block that does
 not fit the device at all.
 
 Every stage of every chunk runs in the library's kernels through the C-ABI (set_state / step / get_state on device
@@ -36,7 +38,7 @@ class HostStepper:
         self.p_ref = p_ref
         self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         self._slots = {}       # (planes, bc_lo, bc_hi, slot) -> (handle, device buffer)
-        self.h2d_bytes = self.d2h_bytes = 0
+        self.h2d_bytes = self.d2h_bytes = self.d2d_bytes = 0
         self._rates, self.rate = None, float("nan")
 
     # where the planes [a, b) of a chunk's block come from: runs of host planes, wrapped around a periodic block
@@ -72,8 +74,9 @@ class HostStepper:
             bc = self.bc[:4] + (bc_lo, bc_hi)
             h = binding.KratosHydro(nx, ny, planes, self.gamma, bc, precision=self.precision, spacing=self.spacing,
                                     stream=self.streams[slot])
-            buf = torch.empty((5, planes, ny, nx), dtype=torch.float64, device="cuda")
-            self._slots[key] = (h, buf)
+            bin_ = torch.empty((5, planes, ny, nx), dtype=torch.float64, device="cuda")    # what was uploaded (kept for the next chunk)
+            bout = torch.empty((5, planes, ny, nx), dtype=torch.float64, device="cuda")   # the chunk block after the step
+            self._slots[key] = (h, bin_, bout)
         return self._slots[key]
 
     def step(self, src, dst, dt):
@@ -87,23 +90,44 @@ class HostStepper:
         plan = self.plan()
         if self._rates is None or self._rates.numel() != len(plan):
             self._rates = torch.zeros(len(plan), dtype=torch.float64, device="cuda")
+        prev = None          # (input buffer, first plane, end plane, event: uploaded) of the previous chunk
+        freed = [None, None]  # per slot: event after which its input buffer may be overwritten (the next chunk has copied from it)
         for i, (z0, z1, a, b, bc_lo, bc_hi) in enumerate(plan):
             slot = i & 1
-            h, buf = self._slot(b - a, bc_lo, bc_hi, slot)
-            with torch.cuda.stream(self.streams[slot]):
-                off = 0
-                for zz, n in self._runs(a, b):
+            stream = self.streams[slot]
+            h, bin_, bout = self._slot(b - a, bc_lo, bc_hi, slot)
+            with torch.cuda.stream(stream):
+                if freed[slot] is not None:
+                    stream.wait_event(freed[slot])
+                # planes the previous chunk has on the device already (its upper overlap = this chunk's lower one) are copied
+                # there; everything else comes up from the host, every plane of the block exactly once per step
+                lo = a
+                if prev is not None and prev[1] <= a < prev[2] and not (a < 0):
+                    pbuf, pa, pb, pev = prev
+                    n = min(pb, b) - a
+                    stream.wait_event(pev)
+                    bin_[:, 0:n].copy_(pbuf[:, a - pa:a - pa + n], non_blocking=True)
+                    lo = a + n
+                    ev = torch.cuda.Event()
+                    ev.record(stream)
+                    freed[slot ^ 1] = ev
+                    self.d2d_bytes += 40 * nx * ny * n
+                off = lo - a
+                for zz, n in self._runs(lo, b):
                     for f in range(5):      # contiguous runs: plain asynchronous copies
-                        buf[f, off:off + n].copy_(src[f, zz:zz + n], non_blocking=True)
+                        bin_[f, off:off + n].copy_(src[f, zz:zz + n], non_blocking=True)
                     off += n
-                h.set_state(buf)
+                    self.h2d_bytes += 40 * nx * ny * n
+                up = torch.cuda.Event()
+                up.record(stream)
+                prev = (bin_, a, b, up)
+                h.set_state(bin_)
                 h.set_reference_pressure(self.p_ref)
                 h.step(dt)
                 h.get_rate(self._rates[i:i + 1])     # CFL rate of the chunk's new state, reduced inside its stage 2
-                h.get_state(buf)
+                h.get_state(bout)
                 for f in range(5):
-                    dst[f, z0:z1].copy_(buf[f, z0 - a:z1 - a], non_blocking=True)
-            self.h2d_bytes += 40 * nx * ny * (b - a)
+                    dst[f, z0:z1].copy_(bout[f, z0 - a:z1 - a], non_blocking=True)
             self.d2h_bytes += 40 * nx * ny * (z1 - z0)
         for s in self.streams:
             s.synchronize()
@@ -116,9 +140,9 @@ class HostStepper:
         return float(cfl) / self.rate
 
     def launch_count(self):
-        return sum(h.launch_count() for h, _ in self._slots.values())
+        return sum(v[0].launch_count() for v in self._slots.values())
 
     def destroy(self):
-        for h, _ in self._slots.values():
-            h.destroy()
+        for v in self._slots.values():
+            v[0].destroy()
         self._slots = {}
