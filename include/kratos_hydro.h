@@ -244,6 +244,49 @@ KRATOS_API int kratos_hydro_set_rate(kratos_hydro_t *h, const double *rate, int 
 KRATOS_API int kratos_hydro_get_reference_pressure(kratos_hydro_t *h, double *p_ref);
 KRATOS_API int kratos_hydro_set_reference_pressure(kratos_hydro_t *h, double p_ref);
 
+/* ---- Conserved totals without any allocation.
+ *
+ * Who this is for.  Everything above works on a handle, and kratos_hydro_create calls cudaMalloc for the handle's state
+ * and work buffers.  Some hosts of this library cannot afford that call, or cannot make it succeed:
+ *   - a simulation framework (Kratos' own mesh manager is one) or a tensor library that has reserved the
+ *     whole device for its own memory pool at start-up: a cudaMalloc issued later by a guest library either fails with
+ *     "out of memory" or takes pages the pool's owner believed it had;
+ *   - code between the steps of a running simulation that must not stall the device: cudaMalloc and cudaFree wait for all
+ *     outstanding work on the device, so one diagnostic call would serialise every stream of the application.
+ * Such a caller keeps the state in its own device memory already.  It can still ask for the conserved totals (the
+ * conservation diagnostic of PAPER.md:232-238: mass, momentum and energy conserved to machine accuracy) with the call
+ * below, which needs no handle and calls neither cudaMalloc, cudaFree nor any library routine that allocates.
+ *
+ * How.  The per-block partial sums that kratos_hydro_totals keeps in a buffer of the handle live here in an array that is
+ * part of the library image itself (a file-scope __device__ array, KRATOS_TOTALS_STATIC_SCRATCH_BYTES = 47 424 bytes).  Every
+ * GPU on which this library has been loaded by the CUDA runtime holds one copy of it until the process exits, whether the
+ * call is ever used or not.  The size is fixed: the grid is capped at 592 thread blocks, each leaving one double-double
+ * per field.
+ *
+ *   U        device pointer, on the calling thread's current device: 5*ncell doubles, U[5][ncell] (the layout at the top
+ *            of this file; only the field stride matters here).  Not modified.
+ *   ncell    1 <= ncell <= KRATOS_TOTALS_STATIC_MAX_CELLS, else KRATOS_ERR_ARG and nothing is launched.
+ *   out      5 doubles, owned by the caller: out_on_device = 1: device pointer on the same device, the call is
+ *            asynchronous on the stream; out_on_device = 0: host pointer, the call synchronises the stream.
+ *   stream   a cudaStream_t passed as void* (NULL: the legacy default stream).
+ * The result is, bit for bit, what kratos_hydro_totals returns for a handle holding the same state (same kernels, same
+ * grid, same order of summation).  Returns KRATOS_OK, KRATOS_ERR_ARG (NULL pointer, ncell out of range, U or a device
+ * `out` that is not device memory of the current device) or KRATOS_ERR_CUDA.
+ *
+ * Things to know.
+ *  - The first call on each device looks up the device address of the scratch array (cudaGetSymbolAddress, which may make the
+ *    runtime load the library's device code onto that GPU).  Make that first call once at start-up, outside any stream
+ *    capture; later calls on that device only launch the two kernels.
+ *  - All calls on one device share the one array.  Nothing in it needs clearing between calls (each call overwrites every
+ *    slot it later reads, whatever an earlier call with another ncell left there), but two calls whose kernels can be on the
+ *    GPU at the same time -- different streams without an ordering between them, or two host threads -- race on it and
+ *    both return garbage.  Order them (one stream, or an event) yourself; the library does not.
+ *  - The call is thread-safe on the host side only in the sense that the one-time set-up is locked. */
+#define KRATOS_TOTALS_STATIC_MAX_CELLS (1LL << 31)  /* 2 147 483 648 cells: an 80 GiB fp64 state */
+#define KRATOS_TOTALS_STATIC_SCRATCH_BYTES 47424
+KRATOS_API int kratos_hydro_totals_static(const double *U, long long ncell, double *out, int out_on_device,
+                                          void *cuda_stream);
+
 /* Message of the last error raised on this thread ("" if none).  Never NULL. */
 KRATOS_API const char *kratos_hydro_last_error(void);
 

@@ -35,6 +35,8 @@ SYMBOLS = [
     "kratos_hydro_push_halo", "kratos_hydro_begin_run", "kratos_hydro_substep", "kratos_hydro_end_run",
     "kratos_hydro_get_rate", "kratos_hydro_set_rate", "kratos_hydro_get_reference_pressure",
     "kratos_hydro_set_reference_pressure",
+    # the totals for callers that may not allocate device memory (no handle)
+    "kratos_hydro_totals_static",
 ]
 
 _lib = None
@@ -128,6 +130,8 @@ def load() -> ctypes.CDLL:
     L.kratos_hydro_last_error.argtypes = []
     L.kratos_hydro_version.restype = ctypes.c_char_p
     L.kratos_hydro_version.argtypes = []
+    L.kratos_hydro_totals_static.restype = i
+    L.kratos_hydro_totals_static.argtypes = [vp, ctypes.c_longlong, vp, i, vp]
     _lib = L
     return L
 
@@ -157,6 +161,43 @@ def _buffer(x):
             raise ValueError("tensor must be contiguous float64")
         return x.data_ptr(), 1 if x.is_cuda else 0, x
     raise TypeError(type(x))
+
+
+TOTALS_STATIC_MAX_CELLS = 1 << 31
+
+
+def totals_static(U, out=None, stream=None, ncell=None):
+    """``kratos_hydro_totals_static``: the five conserved totals of a state that already sits in device memory, for
+    programs that cannot let this library allocate -- the device is wholly owned by their own memory pool, or they
+    are in the middle of a run and cannot take the device-wide wait a ``cudaMalloc`` / ``cudaFree`` brings.  No handle
+    is created; the partial sums go to an array built into the library (shared by all calls on a device: do not let two
+    calls overlap on the GPU).  The first call on a device should be made outside any stream capture.
+
+    ``U``: CUDA tensor, contiguous float64, 5*ncell values (``ncell`` defaults to ``U.numel() // 5``; at most
+    ``TOTALS_STATIC_MAX_CELLS``).  ``out``: None -> a new numpy array of 5 (the call synchronises ``stream``), or a
+    CUDA float64 tensor of 5 on the same device (asynchronous).  ``stream``: a torch.cuda.Stream, a raw cudaStream_t
+    integer, or None for torch's current stream.  Equals ``KratosHydro.totals()`` of the same state bit for bit."""
+    import torch
+    L = load()
+    if not (isinstance(U, torch.Tensor) and U.is_cuda):
+        raise TypeError("U must be a CUDA tensor (the caller owns the state on the device)")
+    ptr, _dev, _keep = _buffer(U)
+    n = U.numel() // 5 if ncell is None else int(ncell)
+    if ncell is None and U.numel() != 5 * n:
+        raise ValueError("state must hold 5*ncell values")
+    if stream is None:
+        stream = torch.cuda.current_stream(U.device)
+    sptr = ctypes.c_void_p(int(getattr(stream, "cuda_stream", stream) or 0))
+    with torch.cuda.device(U.device):
+        if out is None:
+            host = (ctypes.c_double * 5)()
+            _check(L.kratos_hydro_totals_static(ctypes.c_void_p(ptr), n, ctypes.cast(host, ctypes.c_void_p), 0, sptr))
+            return np.array(host[:])
+        optr, odev, _keep2 = _buffer(out)
+        if out.numel() != 5:
+            raise ValueError("out must hold 5 values")
+        _check(L.kratos_hydro_totals_static(ctypes.c_void_p(ptr), n, ctypes.c_void_p(optr), odev, sptr))
+        return out
 
 
 class KratosHydro:

@@ -946,3 +946,88 @@ int kratos_hydro_set_reference_pressure(kratos_hydro_t* h, double p_ref)
     h->pref_valid = true;
     return KRATOS_OK;
 }
+
+// ---------------------------------------------------------------------------------------
+// kratos_hydro_totals_static: the conserved totals for a caller that may not allocate (see the header for who that is).
+//
+// kratos_hydro_totals needs a place for one double-double per field and thread block; a handle gets it from cudaMalloc.
+// Here that place is part of the library image: a file-scope device array, present on every GPU the runtime has loaded
+// this library onto, for as long as the process lives.  Layout: [5][592] dd partial sums, then 8 doubles of which the
+// first 5 receive the finished totals when the caller wants them on the host.
+//
+// Host code must not hand `g_totals_static_scratch` itself to a kernel: in host code that name stands for a host-side
+// shadow object, not for the array on the GPU.  The device address comes from cudaGetSymbolAddress, asked once per
+// device with that device current, and is remembered in g_static_addr[].
+#include <mutex>
+
+namespace {
+
+enum { STATIC_TOT_BLOCKS = 592, STATIC_TAIL_DOUBLES = 8, STATIC_MAX_DEVICES = 64 };
+enum { STATIC_SCRATCH_DOUBLES = 2 * 5 * STATIC_TOT_BLOCKS + STATIC_TAIL_DOUBLES };
+static_assert(sizeof(dd) == 2 * sizeof(double), "dd is two doubles");
+static_assert(sizeof(double) * STATIC_SCRATCH_DOUBLES == KRATOS_TOTALS_STATIC_SCRATCH_BYTES, "header and array disagree");
+
+static __device__ __align__(256) double g_totals_static_scratch[STATIC_SCRATCH_DOUBLES];
+
+std::mutex g_static_mu;
+double* g_static_addr[STATIC_MAX_DEVICES];  // device address of the array on device d; NULL = not asked yet
+
+// Device address of the scratch array on the current device `dev` (first call per device: the look-up).
+int static_scratch_on(int dev, double** out)
+{
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(KRATOS_ERR_ARG, "totals_static: device ordinal %d not supported (< %d)", dev, (int)STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[dev]) {
+        double* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void**)&p, g_totals_static_scratch);
+        if (e != cudaSuccess || !p)
+            return fail(KRATOS_ERR_CUDA, "totals_static: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+        g_static_addr[dev] = p;
+    }
+    *out = g_static_addr[dev];
+    return KRATOS_OK;
+}
+
+// true when p is device (or managed) memory that belongs to device dev
+bool is_memory_of_device(const void* p, int dev)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) && a.device == dev;
+}
+
+}  // namespace
+
+int kratos_hydro_totals_static(const double* U, long long ncell, double* out, int out_on_device, void* cuda_stream)
+{
+    if (!U || !out) return fail(KRATOS_ERR_ARG, "totals_static: NULL argument");
+    if (ncell < 1 || ncell > KRATOS_TOTALS_STATIC_MAX_CELLS)
+        return fail(KRATOS_ERR_ARG, "totals_static: ncell = %lld is outside 1 .. KRATOS_TOTALS_STATIC_MAX_CELLS = %lld",
+                    ncell, (long long)KRATOS_TOTALS_STATIC_MAX_CELLS);
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (!is_memory_of_device(U, dev)) return fail(KRATOS_ERR_ARG, "totals_static: U is not device memory of the current device %d", dev);
+    if (out_on_device && !is_memory_of_device(out, dev))
+        return fail(KRATOS_ERR_ARG, "totals_static: out is not device memory of the current device %d (out_on_device = 1)", dev);
+    double* scratch = nullptr;
+    int rc = static_scratch_on(dev, &scratch);
+    if (rc) return rc;
+
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    // the grid of kratos_hydro_totals (kratos_hydro_create: tot_blocks), so that the sums come out in the same order
+    const int blocks = (int)((ncell + 255) / 256 < STATIC_TOT_BLOCKS ? (ncell + 255) / 256 : STATIC_TOT_BLOCKS);
+    dd* partial = reinterpret_cast<dd*>(scratch);
+    double* tail = scratch + 2 * 5 * STATIC_TOT_BLOCKS;
+    totals_kernel<double><<<dim3(blocks, 5), 256, 0, stream>>>(U, ncell, partial);
+    totals_final_kernel<<<1, 32, 0, stream>>>(partial, blocks, out_on_device ? out : tail);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(KRATOS_ERR_CUDA, "totals_static: launch: %s", cudaGetErrorString(e));
+    if (!out_on_device) {
+        CUDA_TRY(cudaMemcpyAsync(out, tail, sizeof(double) * 5, cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaStreamSynchronize(stream));
+    }
+    return KRATOS_OK;
+}
