@@ -369,8 +369,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": {0: "f32 flux / f64 state", 1: "f64", 2: "f32"}[prec], "data": "synthetic",
         "config": {"workload": wl_name, "grid": [nx, ny, nz], "precision": args.precision,
                    "scheme": "PLM-minmod + HLLC + " + ("van Leer" if vanleer else "Heun"), "kernel": args.kernel, "cfl": pr.cfl, "parallelism": f"replicas x{world}",
-                   "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
-                   if 40 * ncell > 2.5e8 else "state fits L2: no flush between steps (steps are data-dependent)",
+                   "l2": l2_note(ncell, 4 if prec == 2 else 8),
                    "floor_hits": hits},
         "hbm_roofline_frac_step": step_frac,
         "roofline": roofline, "kernels": kern,
@@ -457,14 +456,20 @@ def run_slabs(args):
     barrier()
     w2 = time.time()
     for _ in range(e2e_steps):
-        s.set_state(host)                  # H2D of the whole block from pinned memory, cut into slabs on the device
+        s.set_state(host)                  # H2D from pinned memory: the whole block cut into slabs on the device (one
+                                           # process), or the planes this rank owns only (one process per GPU)
         s.run(pr.cfl, 1, 0.0)
         if world == 1:
             s.get_state_into(host)         # slabs joined on the device, one D2H copy
+            down = 40 * ncell
         else:
             got = s.get_state()
+            down = sum(int(g.size) * 8 for g in got.values())
     barrier()
     e2e_s = replicas.job_time(time.time() - w2)
+    # bytes that crossed the bus per step, summed over the ranks (counted from the copies, not from the grid)
+    moved = s.comm.all_sum([float(s.last_upload_bytes), float(down)])
+    h2d_bytes, d2h_bytes = int(moved[0]), int(moved[1])
     s.destroy()
     if rank != 0:
         if dist is not None:
@@ -499,13 +504,31 @@ def run_slabs(args):
                    "l2": f"state is {5 * 8 * ncell / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)", "floor_hits": hits},
         "hbm_roofline_frac_step": value / world * 200.0 / (peak * 1e9),
         "roofline": roofline, "kernels": kern, "cpu_baseline": None,
-        "e2e": {"value": ncell * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 40 * ncell, "d2h_bytes_per_step": 40 * ncell,
+        "e2e": {"value": ncell * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
                 "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+L2_BYTES = 126e6   # B200
+
+
+def l2_note(ncell, word):
+    """What the config says about the L2: a step touches two copies of the state (Heun: U and the predictor).  Larger than
+    the L2 per copy: every step streams from HBM, no flush needed.  Otherwise part or all of the working set stays on chip
+    between steps (the steps are data-dependent, so nothing can be flushed in between without changing the run): the HBM
+    fraction of such a line is not a statement about HBM."""
+    copy = 5 * word * ncell
+    if copy > L2_BYTES:
+        return f"state is {copy / 1e9:.2f} GB per copy, larger than the 126 MB L2 (no flush needed)"
+    if 2 * copy > L2_BYTES:
+        return (f"state is {copy / 1e6:.0f} MB per copy: one copy fits the 126 MB L2, the step's two do not -- partly on-chip, "
+                "no flush between steps (steps are data-dependent); the HBM fraction is flattered by L2 hits")
+    return (f"on-chip: state is {copy / 1e6:.2f} MB per copy, the whole working set stays in the 126 MB L2; launch-bound, "
+            "the HBM fraction says nothing here")
 
 
 def main():

@@ -136,8 +136,10 @@ class _DistComm:
         # no rank passes this point before every rank's stream has reached it
         import torch
         self._drain(device)
-        dev = device if self.nccl else "cpu"
-        if self._token is None or self._token.device != torch.device(dev):
+        if self._token is None:
+            # created once: NCCL reduces it on this rank's GPU (the device is spelled out -- torch.device("cuda") carries
+            # no index and never compares equal to the "cuda:0" a tensor reports), any other backend on the host
+            dev = torch.device("cuda", torch.cuda.current_device()) if self.nccl else torch.device("cpu")
             self._token = torch.zeros(1, dtype=torch.float32, device=dev)
         self.dist.all_reduce(self._token, group=self.group)
 
@@ -238,17 +240,35 @@ class SlabSolver:
         """U: the state of the WHOLE block, [5, nz, ny, nx] float64 on the host (every rank takes its planes), or
         {rank: local state} for the ranks this process owns."""
         import torch
+        self.last_upload_bytes = 0     # host -> device bytes of this call (this process)
         if isinstance(U, torch.Tensor):
-            # a torch tensor (pinned host memory or device): one copy onto the device, the slabs are cut there
+            nx, ny, nz = self.shape
+            Uv = U.reshape(5, nz, ny, nx)
             with self._ctx():
-                Ud = U.to(self.device, non_blocking=True).reshape(5, self.shape[2], self.shape[1], self.shape[0])
-                for r, b in self.blocks.items():
-                    z0, z1 = self.dec.planes(r)
-                    b.set_state(Ud[:, z0:z1].contiguous())
-                del Ud
+                if U.is_cuda or len(self.blocks) == self.world:
+                    # every plane is wanted on this device: one copy onto it, the slabs are cut there
+                    Ud = Uv.to(self.device, non_blocking=True)
+                    self.last_upload_bytes = 0 if U.is_cuda else U.numel() * 8
+                    for r, b in self.blocks.items():
+                        z0, z1 = self.dec.planes(r)
+                        b.set_state(Ud[:, z0:z1].contiguous())
+                    del Ud
+                else:
+                    # one process per GPU: only the planes this rank owns cross the bus, one contiguous run per field
+                    # (a block that fits only when decomposed is never whole on any one device)
+                    for r, b in self.blocks.items():
+                        z0, z1 = self.dec.planes(r)
+                        part = torch.empty((5, z1 - z0, ny, nx), dtype=torch.float64, device=self.device)
+                        for m in range(5):
+                            part[m].copy_(Uv[m, z0:z1], non_blocking=True)
+                        self.last_upload_bytes += part.numel() * 8
+                        b.set_state(part)
+                        del part
         else:
             for r, b in self.blocks.items():
-                b.set_state(U[r] if isinstance(U, dict) else self.dec.scatter(U, r))
+                loc = U[r] if isinstance(U, dict) else self.dec.scatter(U, r)
+                self.last_upload_bytes += loc.size * 8 if isinstance(loc, np.ndarray) else 0
+                b.set_state(loc)
         # one reference pressure for the whole domain (reading S17): the smallest of the blocks' own choices
         p = min(b.get_reference_pressure() for b in self.blocks.values())
         p = self.comm.all_min_float(p)

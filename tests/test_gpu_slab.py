@@ -156,15 +156,16 @@ def test_state_through_torch_tensors():
 
 
 # --------------------------------------------------------------------------- one process per slab (the deployment layout)
-def _ipc_worker(rank, world, port, shape, bc, nsteps, out):
+def _ipc_worker(rank, world, port, shape, bc, nsteps, out, backend="gloo"):
     import os
     import torch
     import torch.distributed as dist
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
-    dist.init_process_group("gloo", rank=rank, world_size=world)   # (NCCL refuses two ranks on one GPU; the box has one)
+    # gloo: all ranks on GPU 0 (NCCL refuses two ranks on one GPU; the test box has one).  nccl: one GPU per rank.
+    torch.cuda.set_device(rank if backend == "nccl" else 0)
+    dist.init_process_group(backend, rank=rank, world_size=world)
     try:
-        torch.cuda.set_device(0)
         nx, ny, nz = shape
         pr = inputs.random_smooth(nx, ny, nz, seed=31, bc=bc, gamma=1.4)
         s = SlabSolver(nx, ny, nz, pr.gamma, pr.bc)                # distributed: this process owns the slab of its rank
@@ -179,8 +180,24 @@ def _ipc_worker(rank, world, port, shape, bc, nsteps, out):
         dist.destroy_process_group()
 
 
+def _device_count():
+    import torch
+    return torch.cuda.device_count()
+
+
+@pytest.mark.parametrize("shape,bc,world", [((64, 32, 24), (P, P, P, P, P, P), 2), ((32, 32, 21), (F, F, R, R, O, R), 2)])
+def test_one_process_per_gpu_over_nccl(shape, bc, world):
+    """The deployment itself: one process and one GPU per slab, NCCL for the rate maximum and the ordering token (both
+    enqueued on the kernels' stream: no host round trip), the stage kernels' TMA stores landing in the neighbour GPU's
+    ghost arrays over NVLink.  Needs `world` GPUs: skipped on the one-GPU test box, where the gloo test below covers the
+    same calls."""
+    if _device_count() < world:
+        pytest.skip("needs %d CUDA devices, this box has %d" % (world, _device_count()))
+    test_one_process_per_slab_through_cuda_ipc(shape, bc, world, backend="nccl")
+
+
 @pytest.mark.parametrize("shape,bc,world", [((64, 32, 24), (P, P, P, P, P, P), 2), ((32, 32, 21), (F, F, R, R, O, R), 3)])
-def test_one_process_per_slab_through_cuda_ipc(shape, bc, world):
+def test_one_process_per_slab_through_cuda_ipc(shape, bc, world, backend="gloo"):
     """The layout of a multi-GPU run -- one process per slab, the neighbours' ghost arrays mapped through CUDA IPC handles
     (kratos_hydro_ghost_ipc_handle / open_peer), reductions and ordering through the process group -- on the one GPU of the
     test box: the processes share it, no kernel waits for another (the host drains the stream before every collective).
@@ -193,7 +210,7 @@ def test_one_process_per_slab_through_cuda_ipc(shape, bc, world):
         port = sk.getsockname()[1]
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
-    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, shape, bc, nsteps, out)) for r in range(world)]
+    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, shape, bc, nsteps, out, backend)) for r in range(world)]
     for p in procs:
         p.start()
     res = sorted((out.get(timeout=300) for _ in range(world)), key=lambda x: x[0])

@@ -204,7 +204,10 @@ def _worker(rank, world, port, shape, bc, nsteps, out):
         holder["dec"] = SlabDecomposition(nz, world, bc[4], bc[5])
         s = SlabSolver(nx, ny, nz, pr.gamma, pr.bc, make_block=make_block)
         assert s.world == world and s.ranks == [rank]
-        s.set_state(pr.U)
+        # world 3: the whole block as a (host) torch tensor -- a rank must move the planes it owns and no others
+        s.set_state(torch.from_numpy(pr.U) if world == 3 else pr.U)
+        z0, z1 = s.dec.planes(rank)
+        assert s.last_upload_bytes == 5 * 8 * nx * ny * (z1 - z0)
         t = s.run(pr.cfl, nsteps)
         U = s.get_state_global()
         out.put((rank, t, U, s.p_ref, s.totals(), s.cfl_dt(0.4)))
