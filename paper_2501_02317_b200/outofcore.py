@@ -24,7 +24,7 @@ HALO = 4   # planes of dependence of one Heun step: 2 stages x 2 cells
 
 
 class HostStepper:
-    def __init__(self, nx, ny, nz, gamma, bc, chunk=64, precision=binding.PREC_MIXED, p_ref=None):
+    def __init__(self, nx, ny, nz, gamma, bc, chunk=64, precision=binding.PREC_MIXED, p_ref=None, spacing=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("HostStepper needs a CUDA device: the product path has no CPU fallback")
@@ -34,7 +34,11 @@ class HostStepper:
         if nz < 2 * HALO + 1:
             raise ValueError("the block needs more planes than the step's domain of dependence")
         self.chunk = max(1, min(int(chunk), nz))
-        self.spacing = (1.0 / nx, 1.0 / ny, 1.0 / nz)
+        # cell sizes (dx, dy, dz) of the WHOLE block, handed to every chunk's handle: a chunk has fewer planes, not thinner
+        # ones.  Default: the unit box, as for KratosHydro and SlabSolver.
+        self.spacing = (1.0 / nx, 1.0 / ny, 1.0 / nz) if spacing is None else tuple(float(d) for d in spacing)
+        if len(self.spacing) != 3:
+            raise ValueError("spacing = (dx, dy, dz)")
         self.p_ref = p_ref
         self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         self._slots = {}       # (planes, bc_lo, bc_hi, slot) -> (handle, device buffer)

@@ -51,3 +51,31 @@ def test_plan_covers_the_block_once_and_takes_the_halo_along():
     assert sp.plan()[0][2:4] == (-HALO, 16 + HALO) and sp._runs(-HALO, 3) == [(26, 4), (0, 3)]
     assert sp._runs(28, 34) == [(28, 2), (0, 4)]
     sp.destroy()
+
+
+def test_streamed_step_takes_the_callers_cell_sizes():
+    """A block that is not the unit box (dx != 1/nx): the chunk handles must use the whole block's cell sizes.  With the
+    default spacing the streamed step would silently integrate another problem; with the caller's it is the in-core step."""
+    nx, ny, nz = 32, 32, 24
+    spacing = (0.37 / nx, 2.0 / ny, 1.3 / nz)
+    pr = inputs.random_smooth(nx, ny, nz, seed=77, bc=(P, P, R, R, F, O), gamma=1.4)
+    h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=MIXED, spacing=spacing)
+    h.set_state(pr.U)
+    p_ref = h.get_reference_pressure()
+    dt = h.cfl_dt(0.4)
+    h.step(dt)
+    Uin = h.get_state()
+    h.destroy()
+    a = torch.from_numpy(pr.U.copy()).pin_memory()
+    got = {}
+    for name, sp in (("given", spacing), ("default", None)):
+        b = torch.empty_like(a).pin_memory()
+        st = HostStepper(nx, ny, nz, pr.gamma, pr.bc, chunk=7, p_ref=p_ref, spacing=sp)
+        st.step(a, b, dt)
+        st.destroy()
+        got[name] = b.numpy().reshape(Uin.shape).copy()
+    np.testing.assert_array_equal(got["given"], Uin)
+    assert not np.array_equal(got["default"], Uin)
+    Uo = pr.U.copy()
+    oracle.step(Uo, pr.gamma, pr.bc, dt, spacing)
+    assert_parity(got["given"], Uo, MIXED, what="streamed step on a non-unit box")
