@@ -308,9 +308,8 @@ static int flux_divergence_order(const double *U, int nx, int ny, int nz, double
 }
 
 /* ------------------------------------------------------------------------- */
-/* Sec. 3.3 (PAPER.md:262-264): one Heun (RK2) step of length dt.
- *   U1 = U0 + dt L(U0);  U = 1/2 U0 + 1/2 (U1 + dt L(U1))     (predictor enters with weight 1/2)
- * U is updated in place. */
+/* L(U) of Eq. 2 with the paper's default scheme: slope-limited PLM states (Eq. 3) and HLLC fluxes
+ * (Eq. 4-5) at every face of every active axis, differenced over the cell.  Lout: 5*nx*ny*nz doubles. */
 int orc_flux_divergence(const double *U, int nx, int ny, int nz, double gamma, const int bc[6],
                         double dx, double dy, double dz, double *Lout, long long *floor_hits)
 {
@@ -343,6 +342,9 @@ int orc_step_vl(double *U, int nx, int ny, int nz, double gamma, const int bc[6]
     return 0;
 }
 
+/* Sec. 3.3 (PAPER.md:262-264): one Heun (RK2) step of length dt.
+ *   U1 = U0 + dt L(U0);  U = 1/2 U0 + 1/2 (U1 + dt L(U1))     (predictor enters with weight 1/2)
+ * U is updated in place. */
 int orc_step(double *U, int nx, int ny, int nz, double gamma, const int bc[6],
              double dx, double dy, double dz, double dt, long long *floor_hits)
 {

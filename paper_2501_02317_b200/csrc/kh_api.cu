@@ -43,7 +43,7 @@ static int fail(int code, const char* fmt, ...)
     } while (0)
 
 enum { SLOT_STAGE1 = 0, SLOT_STAGE2 = 1, SLOT_OTHER = 2 };
-enum { CFL_MAX_BLOCKS = 148 * 8 };   // p_partial holds 2 * CFL_MAX_BLOCKS doubles: block sums, then block minima
+enum { CFL_MAX_BLOCKS = 1184 };   // a buffer capacity, not an SM count: p_partial holds 2 * CFL_MAX_BLOCKS doubles: block sums, then block minima
 
 struct kratos_hydro {
     Grid g;
@@ -307,7 +307,7 @@ int convert_state(kratos_hydro* h, double* U, int on_device, bool in)
     for (long long o = 0; o < n; o += chunk) {
         const long long m = (n - o < chunk) ? n - o : chunk;
         double* dev = on_device ? U + o : h->stage_buf;
-        const unsigned blocks = (unsigned)((m + 255) / 256 < 148 * 16 ? (m + 255) / 256 : 148 * 16);
+        const unsigned blocks = (unsigned)((m + 255) / 256 < sm_count() * 16 ? (m + 255) / 256 : sm_count() * 16);
         if (in) {
             if (!on_device) CUDA_TRY(cudaMemcpyAsync(dev, U + o, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, h->stream));
             LaunchTimer lt(h, SLOT_OTHER);

@@ -33,6 +33,21 @@ struct Ctrl {
     int pad;
 };
 
+// Number of SMs of the calling thread's current device (148 on B200): what the launch heuristics size their grids by.
+// Asked once per device; falls back to the B200's 148 if the query fails.
+inline int sm_count()
+{
+    static int cached[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (!cached[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached[dev] = n;
+    }
+    return cached[dev];
+}
+
 // Grid description passed by value to every kernel.
 struct Grid {
     int n[3];          // nx, ny, nz
@@ -140,10 +155,11 @@ struct Prim {
 
 // Sec. 3.1: (rho, m, eps) -> (rho, p, v), arithmetic in fp64 in every mode
 // (reading S7: p is a difference of large terms), floors on the primitives only (S6).
-// Returns the number of floor activations (0, 1 or 2).
+// Returns the number of floor activations (0, 1 or 2).  pfl: the pressure floor (mixed precision with a reference
+// pressure: mixed_pressure_floor below; otherwise the plain 1e-30).
 __device__ __forceinline__ int cons_to_prim(double rho, double mx, double my, double mz, double eps,
                                             double gm1, double& p, double& vx, double& vy, double& vz,
-                                            double& rho_out)
+                                            double& rho_out, double pfl = KH_P_FLOOR)
 {
     int hits = 0;
     if (rho < KH_RHO_FLOOR) { rho = KH_RHO_FLOOR; hits++; }
@@ -153,15 +169,28 @@ __device__ __forceinline__ int cons_to_prim(double rho, double mx, double my, do
     vz = mz * ir;
     const double ekin = 0.5 * (mx * vx + my * vy + mz * vz);
     p = gm1 * (eps - ekin);
-    if (p < KH_P_FLOOR) { p = KH_P_FLOOR; hits++; }
+    if (p < pfl) { p = pfl; hits++; }
     rho_out = rho;
     return hits;
+}
+
+// Pressure floor of the one-thread-per-cell kernels (kh_simple.cuh, kh_vanleer.cuh).  Mixed precision (float_t = float,
+// float2_t = double) with a reference pressure: max(1e-30, p_ref 2^-22), the floor of pr::recover (kh_pair.cuh) and of
+// the tiled / TMA / strip kernels, so that floor_hits and the floored state do not depend on which kernel variant served
+// the block (reading S14).  All-fp64 and all-fp32: 1e-30.
+template <typename T, typename S>
+__device__ __forceinline__ S mixed_pressure_floor(const Ctrl* ctrl)
+{
+    if constexpr (sizeof(T) == sizeof(float) && sizeof(S) == sizeof(double))
+        return (S)fmax(KH_P_FLOOR, __dmul_rn(ctrl->p_ref, 0x1p-22));
+    else
+        return (S)KH_P_FLOOR;
 }
 
 // All-fp32 "Single" mode (float2_t = float_t = float): the same recovery on an fp32 state, every
 // operation explicitly rounded (all copies of a cell return the same bits), 1/rho by MUFU.RCP.
 __device__ __forceinline__ int cons_to_prim(float rho, float mx, float my, float mz, float eps, float gm1, float& p,
-                                            float& vx, float& vy, float& vz, float& rho_out)
+                                            float& vx, float& vy, float& vz, float& rho_out, float pfl = (float)KH_P_FLOOR)
 {
     int hits = 0;
     if (rho < (float)KH_RHO_FLOOR) { rho = (float)KH_RHO_FLOOR; hits++; }
@@ -171,7 +200,7 @@ __device__ __forceinline__ int cons_to_prim(float rho, float mx, float my, float
     vz = mul_(mz, ir);
     const float m2 = mul_(fma_(mz, mz, fma_(my, my, mul_(mx, mx))), ir);
     p = mul_(gm1, fma_(-0.5f, m2, eps));
-    if (p < (float)KH_P_FLOOR) { p = (float)KH_P_FLOOR; hits++; }
+    if (p < pfl) { p = pfl; hits++; }
     rho_out = rho;
     return hits;
 }

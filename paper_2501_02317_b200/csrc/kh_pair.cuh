@@ -651,10 +651,10 @@ stage_pair(const double* __restrict__ Uin, const double* U0, double* Uout, Grid 
 inline int auto_zchunk(const Grid& g)
 {
     if (!g.active[2]) return 1;
-    // >= ~12 waves of thread blocks over the 148 SMs (one block per SM), slabs of >= 32 planes
+    // >= ~12 waves of thread blocks over the SMs (148 on B200; one block per SM), slabs of >= 32 planes
     const long long tiles = (long long)((g.n[0] + PTX - 1) / PTX) * ((g.n[1] + PTY - 1) / PTY);
     int chunk = g.n[2];
-    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < (long long)sm_count() * 12) chunk = (chunk + 1) / 2;
     return chunk;
 }
 

@@ -215,7 +215,7 @@ stage_strip(const __grid_constant__ Maps maps, const ST* U0, ST* Uout, Grid g, C
     int s_upd = 0, s_conv = 2, s_issue = 4;
     // U0 of rows 2p-1 and 2p (the rows trip p updates), fetched one trip ahead: 8-byte cp.async copies of the lane's own
     // column into its own entries of sm.u0, a whole trip of latency hidden (the plain loads of the first version, issued and
-    // consumed in the same trip, cost stage 2 two stalled cycles per issued one: profiles/r2a_strip_full.md, long_sb)
+    // consumed in the same trip, cost stage 2 two stalled cycles per issued one: round-2 capture r2a, profiles/history.md: long_sb)
     auto fetch_u0 = [&](int p) {
         if (STAGE != 2) return;
         const bool a = (p > pbeg) && owner, b = (p < pend) && owner;
@@ -386,7 +386,7 @@ inline int auto_rows(const Grid& g)
     // awaited) is paid once per warp.  Slabs shorter than 16 rows are not worth their prologue: small blocks then
     // simply leave SMs idle (they are launch-bound anyway).
     const long long nstrips = (g.n[0] + SW - 1) / SW;
-    const long long slots = 148LL * WARPS * BLOCKS_PER_SM;
+    const long long slots = (long long)sm_count() * WARPS * BLOCKS_PER_SM;
     long long nslabs = slots / nstrips;
     if (nslabs < 1) nslabs = 1;
     int rows = (int)((g.n[1] + nslabs - 1) / nslabs);

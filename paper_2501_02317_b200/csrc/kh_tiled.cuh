@@ -464,10 +464,10 @@ stage_tiled(const double* __restrict__ Uin, const double* U0, double* Uout, Grid
 inline int tiled_auto_zchunk(const Grid& g)
 {
     if (!g.active[2]) return 1;
-    // enough thread blocks for >= ~12 waves over 148 SMs (one block per SM), slabs of >= 16 planes
+    // enough thread blocks for >= ~12 waves over the SMs (148 on B200; one block per SM), slabs of >= 16 planes
     const long long tiles = (long long)((g.n[0] + TX - 1) / TX) * ((g.n[1] + KH_TY_F32 - 1) / KH_TY_F32);
     int chunk = g.n[2];
-    while (chunk > 16 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * KH_BPS_F32 * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 16 && tiles * ((g.n[2] + chunk - 1) / chunk) < (long long)sm_count() * KH_BPS_F32 * 12) chunk = (chunk + 1) / 2;
     return chunk;
 }
 

@@ -1074,11 +1074,11 @@ inline void launch_vl_predict(const StageMaps& sm, const Grid& g, Ctrl* ctrl, in
 
 inline int auto_zchunk(const Grid& g)
 {
-    // >= ~6 waves of thread blocks over the 148 SMs (the tail of the last wave costs ~1 %), slabs of >= 32 planes
+    // >= ~6 waves of thread blocks over the SMs (148 on B200; the tail of the last wave costs ~1 %), slabs of >= 32 planes
     // (every slab converts two extra planes and primes its pipeline: ~3 planes of overhead)
     const long long tiles = (long long)(g.n[0] / PTX) * (g.n[1] / PTY);
     int chunk = g.n[2];
-    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < 148LL * BLOCKS_PER_SM * 6) chunk = (chunk + 1) / 2;
+    while (chunk > 32 && tiles * ((g.n[2] + chunk - 1) / chunk) < (long long)sm_count() * BLOCKS_PER_SM * 6) chunk = (chunk + 1) / 2;
     return chunk;
 }
 
