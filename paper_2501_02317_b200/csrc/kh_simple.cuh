@@ -17,7 +17,7 @@ namespace kh {
 // all-fp32 "Single" mode, where the recovery runs in fp32 as well).
 template <typename T, typename S = double>
 __device__ __forceinline__ Prim<T> load_prim(const S* __restrict__ U, const Grid& g, int ci, int cj, int ck,
-                                             int d, S gm1, int* hits)
+                                             int d, S gm1, int* hits, S pfl = S(KH_P_FLOOR))
 {
     int rx, ry, rz;
     const int si = g.active[0] ? bc_source(ci, g.n[0], g.bc[0], g.bc[1], rx) : (rx = VN_KEEP, 0);
@@ -26,7 +26,7 @@ __device__ __forceinline__ Prim<T> load_prim(const S* __restrict__ U, const Grid
     const long long c = cell_index(g, si, sj, sk);
     S rho, p, vx, vy, vz;
     const int h = cons_to_prim(U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c], gm1, p, vx, vy,
-                               vz, rho);
+                               vz, rho, pfl);
     if (hits) *hits += h;
     vx = apply_vn_rule(vx, rx);
     vy = apply_vn_rule(vy, ry);
@@ -45,7 +45,7 @@ __device__ __forceinline__ Prim<T> load_prim(const S* __restrict__ U, const Grid
 // conserved-field order (rho, m_x, m_y, m_z, eps).
 template <typename T, typename S = double>
 __device__ __noinline__ void face_flux_global(const S* __restrict__ U, const Grid& g, int ci, int cj, int ck,
-                                              int d, T Fout[5])
+                                              int d, T Fout[5], S pfl = S(KH_P_FLOOR))
 {
     const S gm1 = S(g.gamma - 1.0);
     const GasConst<T> gc(g.gamma, 0.0);
@@ -55,7 +55,7 @@ __device__ __noinline__ void face_flux_global(const S* __restrict__ U, const Gri
     for (int s = 0; s < 4; s++) {
         int cc[3] = {c[0], c[1], c[2]};
         cc[d] += s - 2;
-        W[s] = load_prim<T, S>(U, g, cc[0], cc[1], cc[2], d, gm1, nullptr);
+        W[s] = load_prim<T, S>(U, g, cc[0], cc[1], cc[2], d, gm1, nullptr, pfl);
     }
     Prim<T> L, R;
     // left state: cell c-1 plus its half slope; right state: cell c minus its half slope
@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(128) stage_simple(const S* __restrict__ Uin, c
     __shared__ double red[32];
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const double dt = ctrl->dt;
+    const S pfl = mixed_pressure_floor<T, S>(ctrl);
     double rate = 0.0;
     int hits = 0;
     if (c < g.N && dt > 0.0) {
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(128) stage_simple(const S* __restrict__ Uin, c
                 int cc[3] = {i, j, k};
                 cc[d] += side;
                 T F[5];
-                face_flux_global<T, S>(Uin, g, cc[0], cc[1], cc[2], d, F);
+                face_flux_global<T, S>(Uin, g, cc[0], cc[1], cc[2], d, F, pfl);
                 const S sgn = side ? -dtdx : dtdx;
 #pragma unroll
                 for (int m = 0; m < 5; m++) dU[m] = fma_(sgn, (S)F[m], dU[m]);
@@ -111,7 +112,7 @@ __global__ void __launch_bounds__(128) stage_simple(const S* __restrict__ Uin, c
         {
             S p, vx, vy, vz, rho;
             hits = cons_to_prim(Uin[c], Uin[g.N + c], Uin[2 * g.N + c], Uin[3 * g.N + c], Uin[4 * g.N + c],
-                                S(g.gamma - 1.0), p, vx, vy, vz, rho);
+                                S(g.gamma - 1.0), p, vx, vy, vz, rho, pfl);
         }
         S Un[5];
 #pragma unroll

@@ -25,14 +25,14 @@ namespace vl {
 // ---- predictor: first-order flux through the low face of cell (ci,cj,ck) along axis d ----------------------
 template <typename T>
 __device__ __noinline__ void face_flux_const(const double* __restrict__ U, const Grid& g, int ci, int cj, int ck,
-                                             int d, T Fout[5])
+                                             int d, T Fout[5], double pfl)
 {
     const double gm1 = g.gamma - 1.0;
     const GasConst<T> gc(g.gamma, 0.0);
     int cl[3] = {ci, cj, ck};
     cl[d] -= 1;
-    const Prim<T> L = load_prim<T>(U, g, cl[0], cl[1], cl[2], d, gm1, nullptr);
-    const Prim<T> R = load_prim<T>(U, g, ci, cj, ck, d, gm1, nullptr);
+    const Prim<T> L = load_prim<T>(U, g, cl[0], cl[1], cl[2], d, gm1, nullptr, pfl);
+    const Prim<T> R = load_prim<T>(U, g, ci, cj, ck, d, gm1, nullptr, pfl);
     T F[5];
     hllc(L, R, gc, F);
     Fout[0] = F[0];
@@ -48,6 +48,7 @@ __global__ void __launch_bounds__(128) predict(const double* __restrict__ U, T* 
 {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const double dt = ctrl->dt;
+    const double pfl = mixed_pressure_floor<T, double>(ctrl);   // the floor of the TMA predictor in mixed precision
     int hits = 0;
     if (c < g.N && dt > 0.0) {
         const int i = (int)(c % g.n[0]);
@@ -61,7 +62,7 @@ __global__ void __launch_bounds__(128) predict(const double* __restrict__ U, T* 
                 int cc[3] = {i, j, k};
                 cc[d] += side;
                 T F[5];
-                face_flux_const<T>(U, g, cc[0], cc[1], cc[2], d, F);
+                face_flux_const<T>(U, g, cc[0], cc[1], cc[2], d, F, pfl);
                 const double sgn = side ? -hdtdx : hdtdx;
 #pragma unroll
                 for (int m = 0; m < 5; m++) dU[m] += sgn * (double)F[m];
@@ -70,9 +71,10 @@ __global__ void __launch_bounds__(128) predict(const double* __restrict__ U, T* 
         const double gm1 = g.gamma - 1.0;
         double p, vx, vy, vz, rho;
         // floor statistics as in the Heun stages: the recovery of the own cell of U^n, then that of U^{n+1/2}
-        hits = cons_to_prim(U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c], gm1, p, vx, vy, vz, rho);
+        hits = cons_to_prim(U[c], U[g.N + c], U[2 * g.N + c], U[3 * g.N + c], U[4 * g.N + c], gm1, p, vx, vy, vz, rho, pfl);
         hits += cons_to_prim(U[c] + dU[0], U[g.N + c] + dU[1], U[2 * g.N + c] + dU[2], U[3 * g.N + c] + dU[3],
-                             U[4 * g.N + c] + dU[4], gm1, p, vx, vy, vz, rho);
+                             U[4 * g.N + c] + dU[4], gm1, p, vx, vy, vz, rho);   // W^{n+1/2} is stored with the plain
+        // 1e-30 floor, as the TMA predictor stores it (kh_tma.cuh, MODE 1: recover(..., pref = 0))
         Wh[c] = T(rho);
         Wh[g.N + c] = T(p);
         Wh[2 * g.N + c] = T(vx);

@@ -636,6 +636,39 @@ def test_point_blast_with_tiny_background_pressure(kernel):
     assert_parity(Ug, Uo, MIXED)
 
 
+@pytest.mark.parametrize("integrator", [binding.INTEGRATOR_HEUN, binding.INTEGRATOR_VANLEER])
+def test_pressure_floor_is_the_same_in_every_mixed_kernel(integrator):
+    """Reading S14: with a reference pressure the mixed-precision pressure floor is max(1e-30, p_ref 2^-22).  Every kernel
+    variant that can serve a block must apply that same floor, so that floor_hits does not depend on which one did
+    (the one-thread-per-cell kernels floored at 1e-30).  The floor is made to fire by giving the block a
+    reference pressure far above its own: about a third of the cells then lie below p_ref 2^-22.  The step is made so
+    short that the second recovery of the step sees the cells the first one saw (once the floor has fired the variants no
+    longer carry the same pressure: full value in the one-thread-per-cell kernels, fp32 deviation in the others):
+    Heun counts the own cell in both stages, so 2 x below; van Leer counts U^n with this floor and U^{n+1/2} with the
+    plain 1e-30 one (it is stored as full-pressure primitives), so 1 x below."""
+    pr = inputs.random_smooth(64, 32, 12, seed=9, gamma=1.4)
+    rho, m, e = pr.U[0], pr.U[1:4], pr.U[4]
+    pres = (pr.gamma - 1.0) * (e - 0.5 * (m * m).sum(axis=0) / rho)
+    p_ref = float(np.float32(np.quantile(pres, 0.3) * 2.0 ** 22))
+    floor = p_ref * 2.0 ** -22
+    below = int((pres < floor).sum())
+    assert 0.2 * pres.size < below < 0.4 * pres.size
+    assert not np.any(np.abs(pres / floor - 1.0) < 1e-6)       # no cell sits on the threshold
+    heun = integrator == binding.INTEGRATOR_HEUN
+    hits = {}
+    for kernel in ([SIMPLE, TILED, PAIRED, TMA] if heun else [SIMPLE, TMA]):
+        nx, ny, nz = pr.shape
+        h = binding.KratosHydro(nx, ny, nz, pr.gamma, pr.bc, precision=MIXED, kernel=kernel, integrator=integrator)
+        h.set_state(pr.U)
+        h.set_reference_pressure(p_ref)
+        h.step(1e-9 * h.cfl_dt(0.4))
+        h.status()                      # raises if the step left a non-finite state
+        hits[kernel] = h.floor_hits()
+        assert np.isfinite(h.get_state()).all()
+        h.destroy()
+    assert all(v == (2 * below if heun else below) for v in hits.values()), (hits, below)
+
+
 def test_reference_pressure_depends_on_the_state_only():
     """step(dt) after set_state computes the same bits whether or not cfl_dt() or run() was called before on another
     state, and calling cfl_dt() between steps changes nothing (p_ref was hidden state)."""
