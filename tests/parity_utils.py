@@ -8,7 +8,7 @@ Two bounds per conserved field f (BASELINE.json north_star + DESIGN.md section 7
   magnitude where the field is nearly uniform (fp32 rounding errors scale with the magnitude).
   One wrong cell in a block of 10^4 moves the L1 sum by 10^-4 of its own error and would pass the
   first bound; it cannot pass this one.  Measured on the five BASELINE configs at full size
-  (profiles/r2_parity_full_size.md): <= 9.2e-6 mixed, <= 8.4e-14 all-fp64.
+  (profiles/r3_parity_full_size.md; first measured in round 2): <= 9.2e-6 mixed, <= 8.4e-14 all-fp64.
 
 Fields that are identically zero in the oracle (unused momenta) must be identically zero on the GPU.
 """
